@@ -1,0 +1,309 @@
+#!/usr/bin/env python
+"""bench.py -- GLUPS of the two-component Shan-Chen D3Q19 step on B200, against the HBM roofline.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config2|config1|...]
+    python bench.py --impl reference ...        # the CPU oracle, as it stands, on host cores
+
+One "step" is one pass of the whole hot path (moments, force, collide, bounce-back, stream)
+over the whole box: one lb_step(1).  `value` is GLUPS = N_nodes * K / t / 1e9 (PAPER.md:166-171
+Eq. 4) with the state resident in HBM, timed with CUDA events on the stream the kernels are
+launched on.  `e2e` is the same metric through the C ABI with HOST buffers: lb_set_fields
+(H2D) + lb_step(K) + lb_get_moments (D2H) inside one timed region.
+
+The path does not shard (north_star: one GPU, no inter-GPU traffic): --gpus N runs N
+independent replicas, one process per GPU, barrier + max-over-ranks timing ("replicas only",
+DESIGN.md §Multi-GPU).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2112_08264_b200 import workloads as W  # noqa: E402
+
+METRIC = "GLUPS (fp64 two-component D3Q19) on 1 B200; achieved HBM GB/s vs peak"
+WORKLOADS = {f"config{i}": c for i, c in enumerate(W.CONFIGS)}
+ALG_BYTES = {"f64": 608, "f32": 304}     # populations read + written per node per step
+
+
+# ---------------------------------------------------------------------------------------------
+# helpers
+# ---------------------------------------------------------------------------------------------
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def aggregate_over_ranks(ms_local: float, units_local: float, world: int, device=None):
+    """(max time over ranks, total units over ranks).  Works on any torch.distributed backend."""
+    if world == 1:
+        return ms_local, units_local
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    u = torch.tensor([units_local], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.p.terminate()
+        try:
+            out, _ = self.p.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+            out, _ = self.p.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in out.splitlines():
+            c = [v.strip() for v in line.split(",")]
+            if len(c) < 9:
+                continue
+            try:
+                sm.append(float(c[1])), mx.append(float(c[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, c[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def committed_traffic(workload: str, kernel: str):
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(p):
+        return None
+    try:
+        return json.load(open(p)).get(f"{workload}:{kernel}", {}).get("dram_bytes_per_launch")
+    except (ValueError, OSError):
+        return None
+
+
+def time_oracle(cfg, sub, steps, warmup=0):
+    """The oracle, as it stands, single-threaded on a periodic sub-box of the workload's fields."""
+    from oracle import ora
+    sx, sy, sz = sub
+    rr, rb = W.mixture_fields(cfg.nx, cfg.ny, cfg.nz, cfg.seed, chunk=1 << 22) if cfg.n_nodes <= (1 << 24) else (None, None)
+    if rr is None:      # 512^3: generate only the slab we need (same counters, same values)
+        n = np.arange(sz * cfg.ny * cfg.nx, dtype=np.uint64)
+        rr = 1.0 + 0.01 * (2.0 * W.u01(cfg.seed, np.uint64(2) * n) - 1.0)
+        rb = 1.0 + 0.01 * (2.0 * W.u01(cfg.seed, np.uint64(2) * n + np.uint64(1)) - 1.0)
+        rr = rr.reshape(sz, cfg.ny, cfg.nx)[:, :sy, :sx]
+        rb = rb.reshape(sz, cfg.ny, cfg.nx)[:, :sy, :sx]
+    else:
+        rr = rr.reshape(cfg.nz, cfg.ny, cfg.nx)[:sz, :sy, :sx]
+        rb = rb.reshape(cfg.nz, cfg.ny, cfg.nx)[:sz, :sy, :sx]
+    o = ora.Oracle(sx, sy, sz, cfg.tau_r, cfg.tau_b, cfg.G)
+    if cfg.n_spheres:
+        o.set_solid_mask(cfg.solid_mask().reshape(cfg.nz, cfg.ny, cfg.nx)[:sz, :sy, :sx])
+    o.set_fields(np.ascontiguousarray(rr), np.ascontiguousarray(rb))
+    if warmup:
+        o.step(warmup)
+    t0 = time.perf_counter()
+    o.step(steps)
+    dt = time.perf_counter() - t0
+    return sx * sy * sz * steps / dt / 1e9, dt
+
+
+# ---------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle
+# ---------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank, _, world = dist_env()
+    if rank != 0:
+        return 0
+    cfg = WORKLOADS[args.workload]
+    sub = (min(cfg.nx, 64), min(cfg.ny, 32), min(cfg.nz, 32))
+    glups, dt = time_oracle(cfg, sub, args.steps, args.warmup)
+    sample = (f"periodic {sub[0]}x{sub[1]}x{sub[2]} corner of {cfg.name}'s seeded fields, "
+              f"{args.steps} steps after {args.warmup} warm-up")
+    line = {
+        "impl": "reference", "metric": METRIC, "value": glups, "unit": "GLUPS", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "box": [cfg.nx, cfg.ny, cfg.nz], "tau": [cfg.tau_r, cfg.tau_b], "G": cfg.G,
+                   "note": "CPU oracle (oracle/lb_oracle.cpp, g++ -O2 -ffp-contract=off) on a bounded sample"},
+        "cpu_baseline": {"value": glups, "unit": "GLUPS", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": glups, "unit": "GLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------
+# our arm
+# ---------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    from paper_2112_08264_b200 import binding as B
+    from paper_2112_08264_b200.build import build_lib
+
+    rank, local_rank, world = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; this library has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        build_lib()
+    if world > 1:
+        dist.barrier()
+    B.lib()
+
+    cfg = WORKLOADS[args.workload]
+    note = None
+    es = 8 if cfg.dtype == "f64" else 4
+    need = 2 * 38 * cfg.n_nodes * es + 24 * cfg.n_nodes + (1 << 30)
+    free, _total = torch.cuda.mem_get_info(dev)
+    if need > free and args.workload in ("config2", "config3"):
+        note = f"{cfg.name} needs {need >> 30} GiB, {free >> 30} GiB free: fell back to config1"
+        cfg = WORKLOADS["config1"]
+    N = cfg.n_nodes
+    steps, warmup = args.steps, max(args.warmup, 3)
+    dtype = B.LB_F64 if cfg.dtype == "f64" else B.LB_F32
+
+    # inputs: seeded, synthetic, in PINNED host memory (the e2e leg copies from / to these)
+    rr_np, rb_np = cfg.fields()
+    pin = [torch.empty(N, dtype=torch.float64).pin_memory() for _ in range(7)]
+    rr, rb = pin[0].numpy(), pin[1].numpy()
+    rr[:], rb[:] = rr_np, rb_np
+    del rr_np, rb_np
+    outs = [p.numpy() for p in pin[2:7]]
+    mask = cfg.solid_mask()
+
+    stream = torch.cuda.Stream(device=dev)
+    box = B.Box(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype, cuda_stream=stream.cuda_stream)
+    kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS}[args.kernel]
+    box.set_kernel(kernel)
+    if mask is not None:
+        box.set_solid_mask(mask)
+    box.set_fields(rr, rb)
+    kname = B.lb_kernel_name(box.h) if hasattr(B, "lb_kernel_name") else args.kernel
+
+    # ---- device-resident timing: K steps between two events on the launching stream ----
+    box.step(warmup)
+    box.sync()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize(dev)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = box.launch_count()
+    e0.record(stream)
+    box.step(steps)
+    e1.record(stream)
+    e1.synchronize()
+    torch.cuda.synchronize(dev)
+    if world > 1:
+        dist.barrier()
+    launches = box.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    ms_max, units = aggregate_over_ranks(ms, float(N) * steps, world, dev)
+    glups = units / (ms_max * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with host buffers ----
+    box.sync()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    box.set_fields(rr, rb)                      # H2D: 2 fields of N doubles
+    box.step(steps)
+    B.lb_get_moments(box.h, N, outs)            # D2H: 5 fields of N doubles (synchronises)
+    e2e_s = time.perf_counter() - t0
+    e2e_ms_max, _ = aggregate_over_ranks(e2e_s * 1e3, 0.0, world, dev)
+    e2e_glups = units / (e2e_ms_max * 1e-3) / 1e9
+    mass_chk = float(outs[0].sum() + outs[1].sum())
+
+    if rank != 0:
+        box.close()
+        return 0
+
+    peak, peak_src = measured_peak()
+    alg = ALG_BYTES[cfg.dtype]
+    per_launch_ms = ms / max(launches, 1) * (launches / steps)      # = ms / steps: whole step (1 kernel on the one-pass path)
+    achieved = alg * N / (per_launch_ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": glups, "unit": "GLUPS", "n_gpus": world, "steps": steps, "warmup": warmup,
+        "ms_per_step": ms_max / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": cfg.dtype, "data": "synthetic",
+        "config": {"workload": cfg.name, "box": [cfg.nx, cfg.ny, cfg.nz], "tau": [cfg.tau_r, cfg.tau_b], "G": cfg.G,
+                   "solid_spheres": cfg.n_spheres, "kernel": kname, "launches_per_step": launches / steps,
+                   "l2": f"state {2 * 38 * N * es / 2**30:.1f} GiB >> 126 MB L2, no flush needed",
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "diagnostics_in_step": False,
+                   **({"note": note} if note else {})},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": committed_traffic(cfg.name, kname), "peak_source": peak_src,
+                     "algorithmic_bytes_per_node": alg, "kernel_ms": per_launch_ms,
+                     "kernel": "whole step" if launches != steps else "fused one-pass step kernel"},
+        "e2e": {"value": e2e_glups, "unit": "GLUPS", "h2d_bytes_per_step": 2 * N * 8 / steps,
+                "d2h_bytes_per_step": 5 * N * 8 / steps, "seconds": e2e_s, "mass_check": mass_chk,
+                "calls": "lb_set_fields(host) + lb_step(K) + lb_get_moments(host)"},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    if not args.no_cpu_baseline:
+        sub = (min(cfg.nx, 128), min(cfg.ny, 128), min(cfg.nz, 64))
+        cpu_steps = 12
+        cg, cdt = time_oracle(cfg, sub, cpu_steps)
+        line["cpu_baseline"] = {"value": cg, "unit": "GLUPS", "cores": 1, "kind": "oracle", "seconds": cdt,
+                                "sample": f"periodic {sub[0]}x{sub[1]}x{sub[2]} corner of {cfg.name}'s seeded fields, {cpu_steps} steps"}
+    box.close()
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS))
+    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    return run_reference(args) if args.impl == "reference" else run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,134 @@
+/* lb.h -- C ABI of the B200-native two-component Shan-Chen D3Q19 lattice-Boltzmann library.
+ *
+ * One library, one GPU, one opaque context per simulation box.  Every step of the hot
+ * path (moments, Shan-Chen force, BGK collision with forcing, halfway bounce-back,
+ * periodic streaming, diagnostics) runs in hand-written sm_100a CUDA kernels behind
+ * these calls.  There is no CPU fallback: with no CUDA device every call that touches
+ * the device fails with LB_ECUDA.
+ *
+ * Citations: PAPER.md = /root/reference/PAPER.md (LBcuda, arXiv 2112.08264);
+ * S1..S14 = the readings of SURVEY.md 8(c), repeated in DESIGN.md "Readings".
+ *
+ * CONVENTIONS
+ *   Box        nx*ny*nz nodes, periodic on all three axes (section 5).
+ *   Node index n = x + nx*(y + ny*z); every array argument is dense, x fastest, no
+ *              padding.  N = nx*ny*nz.
+ *   Components k = 0 "red", k = 1 "blue".
+ *   Directions i = 0..18, D3Q19, numbered (reading S1):
+ *              0:(0,0,0)  1:(+x) 2:(-x) 3:(+y) 4:(-y) 5:(+z) 6:(-z)
+ *              7:(+x+y) 8:(-x-y) 9:(+x-y) 10:(-x+y)
+ *              11:(+x+z) 12:(-x-z) 13:(+x-z) 14:(-x+z)
+ *              15:(+y+z) 16:(-y-z) 17:(+y-z) 18:(-y+z);  opp(i) = i+1 (i odd), i-1 (i even >= 2).
+ *   Pointers   every pointer argument is a caller-owned HOST array (pageable or pinned).
+ *              The library copies; it never keeps a caller pointer after the call returns.
+ *              All device state is owned by the context; its layout is private.
+ *   Values     the ABI speaks double for both LB_F64 and LB_F32 contexts; an LB_F32 context
+ *              rounds to float on the way in and widens on the way out.
+ *   Errors     lb_create* return NULL on failure; all other calls return LB_OK or a negative
+ *              code; lb_last_error() holds a message for the calling thread.  No exception
+ *              crosses the boundary.
+ *   Ordering   lb_step only enqueues work on the context's stream and may return before the
+ *              GPU finishes; every getter synchronises that stream.
+ *   Threads    one context may be used from one thread at a time.
+ */
+#ifndef LB_B200_H
+#define LB_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lb_ctx lb_ctx;          /* opaque; owned by the library */
+
+enum { LB_OK = 0, LB_EINVAL = -1, LB_ENOMEM = -2, LB_ECUDA = -3, LB_ESTATE = -4 };
+enum { LB_F64 = 0, LB_F32 = 1 };
+enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2 };
+
+/* Create a context for an nx*ny*nz periodic box holding two fluids with BGK
+ * relaxation times tau_r, tau_b (Eq. 1; omega_k = 1/tau_k) coupled by the
+ * Shan-Chen constant G (reading S2: F^k(x) = -G psi^k(x) sum_{i=1..18} w_i psi^kbar(x+c_i) c_i,
+ * psi = rho (S3), w_i the lattice weights of PAPER.md:393-398; G > 0 repels).
+ * fp64 populations, the library's own stream.
+ * NULL (LB_EINVAL) if a dimension is < 1, tau <= 0.5 or not finite (Eq. 2, PAPER.md:84-86,
+ * needs 0 < omega < 2), or G is not finite; NULL (LB_ENOMEM / LB_ECUDA) if device memory or
+ * the device is not available.  Device memory: 2 population buffers of 38*N values plus
+ * about 17 bytes per node. */
+lb_ctx* lb_create(int nx, int ny, int nz, double tau_r, double tau_b, double G);
+
+/* Same, with the population type (LB_F64 / LB_F32: "fp32 populations and fields", all
+ * arithmetic in that type) and, if cuda_stream != NULL, a caller-owned cudaStream_t on
+ * which all the context's work is enqueued (e.g. a torch stream); the caller keeps that
+ * stream alive until lb_destroy. */
+lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double G,
+                     int dtype, void* cuda_stream);
+
+/* Release the context and all its device memory.  lb_destroy(NULL) is a no-op. */
+void lb_destroy(lb_ctx* ctx);
+
+/* Initialise both fluids at local equilibrium (Eq. 10, c_s^2 = 1/3):
+ * f_i^k(x) = f_i^eq(rho^k(x), u(x)).  rho_r, rho_b: N doubles each (required).
+ * ux, uy, uz: N doubles each, or all three NULL for u = 0.  Solid nodes get exactly 0 (S8).
+ * LB_EINVAL on NULL rho pointers or a partial velocity triple. */
+int lb_set_fields(lb_ctx* ctx, const double* rho_r, const double* rho_b,
+                  const double* ux, const double* uy, const double* uz);
+
+/* Static solid nodes (nodes inside particles, "no computation is
+ * performed"): N bytes, nonzero = solid.  May be called before or after lb_set_fields; either
+ * way solid-node populations are exactly 0 afterwards (S8).  Fluid->solid links get halfway
+ * bounce-back with the wall at rest (Eq. 23-24 with u_b = 0); a solid
+ * neighbour contributes psi = 0 to the force sum (S7). */
+int lb_set_solid_mask(lb_ctx* ctx, const unsigned char* mask);
+
+/* Restart / arbitrary state: 38*N doubles, [k][i][z][y][x].  Solid nodes are zeroed. */
+int lb_set_populations(lb_ctx* ctx, const double* f);
+
+/* Advance nsteps time steps.  One step, for every fluid node x (order of PAPER.md:128-138:
+ * collide -> bounce-back -> stream):
+ *   rho^k = sum_i f_i^k, j^k = sum_i f_i^k c_i                          (Eq. 6-7)
+ *   u'    = sum_k omega_k j^k / sum_k omega_k rho^k                     (S4; Eq. 7 when tau_r = tau_b)
+ *   du^k  = -G sum_{i=1..18} w_i rho^kbar((x+c_i) mod box) c_i          (S2, S3, S6, S7)
+ *   f*_i  = (1-omega_k) f_i + omega_k feq_i(rho^k,u') + feq_i(rho^k,u'+du^k) - feq_i(rho^k,u')   (Eq. 1 + S5)
+ *   x+c_i solid: f_opp(i)^k(x,t+1) = f*_i  else  f_i^k((x+c_i) mod box, t+1) = f*_i              (Eq. 23-24; Eq. 5)
+ * Solid nodes keep 0.  LB_EINVAL if nsteps < 0; LB_ESTATE before lb_set_fields /
+ * lb_set_populations; LB_ECUDA on a launch failure.  Asynchronous. */
+int lb_step(lb_ctx* ctx, int nsteps);
+
+/* Copy out all populations: 38*N doubles, [k][i][z][y][x].  Synchronises. */
+int lb_get_populations(lb_ctx* ctx, double* f);
+
+/* rho^k (Eq. 6) and the barycentric velocity u = sum_k j^k / sum_k rho^k (Eq. 7) of the current
+ * state; N doubles each; any pointer may be NULL to skip that field.  Solid nodes and nodes
+ * with zero total density report 0.  Synchronises. */
+int lb_get_moments(lb_ctx* ctx, double* rho_r, double* rho_b, double* ux, double* uy, double* uz);
+
+/* Bounce-back link set: N 32-bit words; bit i of links[n] is set iff node n is fluid and
+ * (n + c_i) mod box is solid.  Integer work: exactly one right answer.  Synchronises. */
+int lb_get_link_mask(lb_ctx* ctx, unsigned int* links);
+
+/* Per-component mass M^k = sum_x rho^k and total momentum P = sum_x sum_k j^k over fluid nodes
+ * of the current state (warp-shuffle + fixed-order block reduction: deterministic).
+ * Accumulated in double for both dtypes.  Synchronises. */
+int lb_get_diagnostics(lb_ctx* ctx, double mass[2], double momentum[3]);
+
+/* Choose the time-step kernel: LB_KERNEL_TWOPASS = density pass + fused collide/stream pass
+ * (reads the populations twice per step); LB_KERNEL_ONEPASS = single fused pass that
+ * reads and writes every population once per step; LB_KERNEL_AUTO (default) = ONEPASS when
+ * the box shape allows it, else TWOPASS.  LB_EINVAL if the box shape does not allow `kind`. */
+int lb_set_kernel(lb_ctx* ctx, int kind);
+
+/* Number of kernel launches this context has enqueued so far (for bench.py's gpu_launches). */
+long long lb_launch_count(const lb_ctx* ctx);
+
+/* Block until all work enqueued on the context's stream has finished. */
+int lb_sync(lb_ctx* ctx);
+
+/* Message for the last failure on the calling thread ("" if none). */
+const char* lb_last_error(void);
+
+/* Library version string. */
+const char* lb_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LB_B200_H */

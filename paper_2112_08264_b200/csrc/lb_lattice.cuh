@@ -1,0 +1,85 @@
+// lb_lattice.cuh -- D3Q19 constants and the per-node collision arithmetic of the CUDA path.
+// (The CPU oracle has its own, separately written tables; nothing here is shared with it.)
+//
+// Direction numbering = include/lb.h (reading S1).  Directions come in opposite pairs
+// (2p+1, 2p+2), p = 0..8, which lets a pair share its (c.u)^2 term.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace lb {
+
+constexpr int Q = 19;
+constexpr int NPOP = 2 * Q;          // two components
+
+// c_i of the ODD member of pair p (direction 2p+1); the even member is its negative.
+__host__ __device__ constexpr int pair_cx(int p) { return (p == 0 || p == 3 || p == 4 || p == 5 || p == 6) ? 1 : 0; }
+__host__ __device__ constexpr int pair_cy(int p) { return (p == 1 || p == 3 || p == 7 || p == 8) ? 1 : (p == 4 ? -1 : 0); }
+__host__ __device__ constexpr int pair_cz(int p) { return (p == 2 || p == 5 || p == 7) ? 1 : ((p == 6 || p == 8) ? -1 : 0); }
+// pairs: 0:(+x) 1:(+y) 2:(+z) 3:(+x+y) 4:(+x-y) 5:(+x+z) 6:(+x-z) 7:(+y+z) 8:(+y-z)
+
+__host__ __device__ constexpr int dir_cx(int i) { return i == 0 ? 0 : ((i & 1) ? pair_cx((i - 1) / 2) : -pair_cx((i - 2) / 2)); }
+__host__ __device__ constexpr int dir_cy(int i) { return i == 0 ? 0 : ((i & 1) ? pair_cy((i - 1) / 2) : -pair_cy((i - 2) / 2)); }
+__host__ __device__ constexpr int dir_cz(int i) { return i == 0 ? 0 : ((i & 1) ? pair_cz((i - 1) / 2) : -pair_cz((i - 2) / 2)); }
+__host__ __device__ constexpr int dir_opp(int i) { return i == 0 ? 0 : ((i & 1) ? i + 1 : i - 1); }
+
+// Lattice weights: 1/3 rest, 1/18 axis (pairs 0-2), 1/36 diagonal (pairs 3-8).
+template <typename T> __host__ __device__ constexpr T w_rest() { return T(1.0 / 3.0); }
+template <typename T> __host__ __device__ constexpr T w_pair(int p) { return p < 3 ? T(1.0 / 18.0) : T(1.0 / 36.0); }
+
+// rho = sum_i f_i and j = sum_i f_i c_i of one component (Eq. 6-7).
+template <typename T>
+__device__ __forceinline__ void moments19(const T (&f)[Q], T& rho, T& jx, T& jy, T& jz) {
+    T r = f[0], x = T(0), y = T(0), z = T(0);
+#pragma unroll
+    for (int p = 0; p < 9; ++p) {
+        const T a = f[2 * p + 1], b = f[2 * p + 2];
+        r += a + b;
+        const T d = a - b;
+        if (pair_cx(p) > 0) x += d; else if (pair_cx(p) < 0) x -= d;
+        if (pair_cy(p) > 0) y += d; else if (pair_cy(p) < 0) y -= d;
+        if (pair_cz(p) > 0) z += d; else if (pair_cz(p) < 0) z -= d;
+    }
+    rho = r; jx = x; jy = y; jz = z;
+}
+
+// BGK collision with exact-difference forcing (Eq. 1; Eq. 10, PAPER.md:338-342;
+// reading S5), in place:
+//   f*_i = (1-om) f_i + om feq_i(rho,u) + feq_i(rho,u+du) - feq_i(rho,u)
+//        = omc f_i + [ feq_i(rho,ue) - omc feq_i(rho,u) ],   omc = 1-om, ue = u+du.
+// With s(v) = 1 - 1.5 v.v + 4.5 (c.v)^2 the pair (i, opp i) shares s; they differ in +-3 c.v.
+// omc is a run-time value; nothing here specialises tau = 1.
+template <typename T>
+__device__ __forceinline__ void collide19(T (&f)[Q], T rho, T omc, T ux, T uy, T uz, T ex, T ey, T ez) {
+    const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    const T ae = T(1) - T(1.5) * (ex * ex + ey * ey + ez * ez);
+    f[0] = omc * f[0] + w_rest<T>() * rho * (ae - omc * a0);
+#pragma unroll
+    for (int p = 0; p < 9; ++p) {
+        const T cu = T(pair_cx(p)) * ux + T(pair_cy(p)) * uy + T(pair_cz(p)) * uz;
+        const T ce = T(pair_cx(p)) * ex + T(pair_cy(p)) * ey + T(pair_cz(p)) * ez;
+        const T wr = w_pair<T>(p) * rho;
+        const T s0 = a0 + T(4.5) * cu * cu;
+        const T se = ae + T(4.5) * ce * ce;
+        const T sym = wr * (se - omc * s0);
+        const T asym = (T(3) * wr) * (ce - omc * cu);
+        f[2 * p + 1] = omc * f[2 * p + 1] + (sym + asym);
+        f[2 * p + 2] = omc * f[2 * p + 2] + (sym - asym);
+    }
+}
+
+// Eq. 10 for all 19 directions.
+template <typename T>
+__device__ __forceinline__ void equilibrium19(T (&f)[Q], T rho, T ux, T uy, T uz) {
+    const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    f[0] = w_rest<T>() * rho * a0;
+#pragma unroll
+    for (int p = 0; p < 9; ++p) {
+        const T cu = T(pair_cx(p)) * ux + T(pair_cy(p)) * uy + T(pair_cz(p)) * uz;
+        const T wr = w_pair<T>(p) * rho;
+        const T s0 = a0 + T(4.5) * cu * cu;
+        f[2 * p + 1] = wr * (s0 + T(3) * cu);
+        f[2 * p + 2] = wr * (s0 - T(3) * cu);
+    }
+}
+
+}  // namespace lb
