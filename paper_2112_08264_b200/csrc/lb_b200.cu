@@ -7,12 +7,14 @@
 #include <cmath>
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
 
 #include "../../include/lb.h"
 #include "lb_lattice.cuh"
+#include "lb_onepass.cuh"
 
 using namespace lb;
 
@@ -317,7 +319,45 @@ int zero_solids_both(lb_ctx* c) {
     return LB_OK;
 }
 
-bool onepass_ok(const lb_ctx*) { return false; }      // replaced when lb_onepass.cuh lands
+// ----------------------------------------------------------------------------------------
+// one-pass time step (lb_onepass.cuh): boxes whose x, y sides are multiples of the 32 x 8 tile
+// ----------------------------------------------------------------------------------------
+constexpr int OP_TX = 32, OP_TY = 8;
+constexpr int OP_RESIDENT_CTAS = 148 * 2;
+
+bool onepass_ok(const lb_ctx* c) { return c->nx % OP_TX == 0 && c->ny % OP_TY == 0; }
+
+// planes per CTA: long enough to amortise the 2-plane density prologue, short enough that the
+// grid is many waves of the resident CTAs; a divisor of nz when one is close.
+int onepass_zc(const lb_ctx* c) {
+    if (const char* e = std::getenv("LB_ONEPASS_ZC")) { const int v = std::atoi(e); if (v >= 1) return v < c->nz ? v : c->nz; }
+    const long long tiles = (long long)(c->nx / OP_TX) * (c->ny / OP_TY);
+    const long long chunks_wanted = (OP_RESIDENT_CTAS * 6 + tiles - 1) / tiles;
+    long long zc = c->nz / (chunks_wanted > 0 ? chunks_wanted : 1);
+    if (zc > 64) zc = 64;
+    if (zc < 16) zc = 16;
+    if (zc > c->nz) zc = c->nz;
+    for (long long d = zc; d >= (zc + 1) / 2; --d)
+        if (c->nz % d == 0) return int(d);
+    return int(zc);
+}
+
+template <typename T>
+int step_onepass(lb_ctx* c) {
+    const T* f = static_cast<const T*>(c->f[c->cur]);
+    T* g = static_cast<T*>(c->f[c->cur ^ 1]);
+    const int zc = onepass_zc(c);
+    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + zc - 1) / zc);
+    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
+    if (c->has_solid)
+        k_step_onepass<T, true, OP_TX, OP_TY><<<grid, OP_TX * OP_TY, 0, c->stream>>>(f, g, c->links, c->NP, c->nx, c->ny, c->nz, zc, om_r, om_b, G);
+    else
+        k_step_onepass<T, false, OP_TX, OP_TY><<<grid, OP_TX * OP_TY, 0, c->stream>>>(f, g, nullptr, c->NP, c->nx, c->ny, c->nz, zc, om_r, om_b, G);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    c->cur ^= 1;
+    return LB_OK;
+}
 
 int resolve_kernel(lb_ctx* c, int kind) {
     if (kind == LB_KERNEL_AUTO) return onepass_ok(c) ? LB_KERNEL_ONEPASS : LB_KERNEL_TWOPASS;
@@ -495,7 +535,9 @@ int lb_step(lb_ctx* c, int nsteps) {
     if (nsteps < 0) return fail(LB_EINVAL, "nsteps must be >= 0");
     if (!c->have_fields) return fail(LB_ESTATE, "lb_step before lb_set_fields / lb_set_populations");
     for (int s = 0; s < nsteps; ++s) {
-        const int rc = c->dtype == LB_F64 ? step_twopass<double>(c) : step_twopass<float>(c);
+        int rc;
+        if (c->kernel == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);
+        else rc = c->dtype == LB_F64 ? step_twopass<double>(c) : step_twopass<float>(c);
         if (rc != LB_OK) return rc;
     }
     return LB_OK;
