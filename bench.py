@@ -106,14 +106,18 @@ def measured_peak():
 
 
 def committed_traffic(workload: str, kernel: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/traffic.csv), if any."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     if not os.path.exists(p):
         return None
     try:
-        return json.load(open(p)).get(f"{workload}:{kernel}", {}).get("dram_bytes_per_launch")
-    except (ValueError, OSError):
-        return None
+        import csv
+        for row in csv.DictReader(open(p)):
+            if row["workload"] == workload and row["kernel"] == kernel:
+                return float(row["dram_bytes_per_launch"])
+    except (ValueError, OSError, KeyError):
+        pass
+    return None
 
 
 def time_oracle(cfg, sub, steps, warmup=0):
