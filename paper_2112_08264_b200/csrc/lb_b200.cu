@@ -2,6 +2,11 @@
 // ("two-pass") kernels that work for any box shape.  The bandwidth-optimised one-pass step
 // lives in lb_onepass.cuh.  sm_100a only; there is no CPU path in this file or anywhere in
 // the library.
+//
+// Device state ("h-state", see lb_onepass.cuh): the population buffer f[cur] holds the
+// post-collision, not yet streamed values h of the previous step; every reader streams while it
+// reads (pull).  The ABI speaks f (streamed populations at their nodes, Eq. 5): k_unstream /
+// k_stream convert on the way in / out.  They are pure moves, so set -> get is bit-exact.
 #include <cuda_runtime.h>
 
 #include <cmath>
@@ -29,14 +34,20 @@ struct lb_ctx {
     double tau[2], G;
     cudaStream_t stream;
     bool own_stream;
-    void* f[2];        // ping-pong population buffers, [k][i][NP]
-    int cur;           // f[cur] holds time t
-    void* rho;         // [k][NP] densities (two-pass path and getters)
+    void* f[2];        // ping-pong population buffers, [k][i][NP]; f[cur] = h-state, f[cur^1] = scratch
+    int cur;
+    // density of the CURRENT time level as the four single-writer arrays of lb_onepass.cuh, ping-pong.
+    // rho_x / rho_y / rho_xy exist only when the box takes the one-pass tile.
+    void* rho_in[2]; void* rho_x[2]; void* rho_y[2]; void* rho_xy[2];
+    long long s_x, s_y, s_xy;   // component strides (elements) of the edge arrays
+    int rcur;
+    bool rho_valid;    // rho_*[rcur] holds the density of the state in f[cur]
     unsigned int* links;   // N words: bit i = neighbour i solid, bit 31 = this node solid
     bool has_solid;
     bool have_fields;
     int kernel;        // resolved LB_KERNEL_*
     int kernel_req;
+    int zc;            // planes per CTA of the one-pass kernel
     double* stage;     // device staging, STAGE_NODES * 5 doubles
     double* diag_part; // [DIAG_BLOCKS][5]
     double* diag_out;  // [5]
@@ -48,6 +59,7 @@ namespace {
 constexpr long long STAGE_NODES = 1ll << 22;
 constexpr int DIAG_BLOCKS = 148 * 8;
 constexpr unsigned SOLID_BIT = 1u << 31;
+constexpr int OP_TX = 32, OP_TY = 8;
 
 thread_local std::string g_err;
 
@@ -66,6 +78,32 @@ size_t esize(const lb_ctx* c) { return c->dtype == LB_F64 ? 8 : 4; }
 
 template <typename T> __device__ __forceinline__ T* plane(T* f, long long NP, int k, int i) { return f + (long long)(k * Q + i) * NP; }
 template <typename T> __device__ __forceinline__ const T* plane(const T* f, long long NP, int k, int i) { return f + (long long)(k * Q + i) * NP; }
+
+// periodic neighbour offsets of node n, any box shape
+struct Nbr {
+    long long o[3][3];    // o[0][dx+1] x offsets, o[1][dy+1] row offsets, o[2][dz+1] plane offsets
+    __device__ __forceinline__ long long at(int dx, int dy, int dz) const { return o[0][dx + 1] + o[1][dy + 1] + o[2][dz + 1]; }
+};
+__device__ __forceinline__ Nbr neighbours(long long n, int nx, int ny, int nz) {
+    const int x = int(n % nx), y = int((n / nx) % ny), z = int(n / ((long long)nx * ny));
+    Nbr b;
+    b.o[0][0] = x == 0 ? nx - 1 : x - 1; b.o[0][1] = x; b.o[0][2] = x == nx - 1 ? 0 : x + 1;
+    b.o[1][0] = (long long)nx * (y == 0 ? ny - 1 : y - 1); b.o[1][1] = (long long)nx * y; b.o[1][2] = (long long)nx * (y == ny - 1 ? 0 : y + 1);
+    const long long pl = (long long)nx * ny;
+    b.o[2][0] = pl * (z == 0 ? nz - 1 : z - 1); b.o[2][1] = pl * z; b.o[2][2] = pl * (z == nz - 1 ? 0 : z + 1);
+    return b;
+}
+
+// the 19 populations of component k arriving at fluid node n: f_i(x) = h_i(x - c_i) (Eq. 5), or
+// h_opp(i)(x) when x - c_i is solid (halfway bounce-back, Eq. 23-24 with u_b = 0).  lk = links[n].
+template <typename T>
+__device__ __forceinline__ void pull19(const T* __restrict__ h, long long NP, int k, long long n, const Nbr& b, unsigned lk, T (&fk)[Q]) {
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+        const bool bounce = i > 0 && (lk >> dir_opp(i) & 1u);
+        fk[i] = bounce ? plane(h, NP, k, dir_opp(i))[n] : plane(h, NP, k, i)[b.at(-dir_cx(i), -dir_cy(i), -dir_cz(i))];
+    }
+}
 
 // ----------------------------------------------------------------------------------------
 // setup / transfer kernels (not on the hot path)
@@ -96,6 +134,51 @@ __global__ void k_zero_solids(T* __restrict__ f, long long NP, long long N, cons
     if (n >= N || !(links[n] & SOLID_BIT)) return;
 #pragma unroll
     for (int q = 0; q < NPOP; ++q) f[(long long)q * NP + n] = T(0);
+}
+
+// f (streamed populations at their nodes) -> h-state: h_j(y) = f_j(y + c_j), or f_opp(j)(y) when
+// y + c_j is solid (so that pulling h gives back exactly f).  Solid nodes hold 0.  links may be NULL.
+template <typename T>
+__global__ void __launch_bounds__(256) k_unstream(const T* __restrict__ f, T* __restrict__ h, const unsigned* __restrict__ links,
+                                                  long long NP, int nx, int ny, int nz) {
+    const long long N = (long long)nx * ny * nz;
+    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    const unsigned lk = links ? links[n] : 0u;
+    const Nbr b = neighbours(n, nx, ny, nz);
+#pragma unroll
+    for (int k = 0; k < 2; ++k)
+#pragma unroll
+        for (int j = 0; j < Q; ++j) {
+            T v;
+            if (lk & SOLID_BIT) v = T(0);
+            else if (j > 0 && (lk >> j & 1u)) v = plane(f, NP, k, dir_opp(j))[n];
+            else v = plane(f, NP, k, j)[b.at(dir_cx(j), dir_cy(j), dir_cz(j))];
+            plane(h, NP, k, j)[n] = v;
+        }
+}
+
+// h-state -> f: the streaming step itself (Eq. 5 / Eq. 23-24), written out for the getters.
+template <typename T>
+__global__ void __launch_bounds__(256) k_stream(const T* __restrict__ h, T* __restrict__ f, const unsigned* __restrict__ links,
+                                                long long NP, int nx, int ny, int nz) {
+    const long long N = (long long)nx * ny * nz;
+    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    const unsigned lk = links ? links[n] : 0u;
+    const Nbr b = neighbours(n, nx, ny, nz);
+#pragma unroll
+    for (int k = 0; k < 2; ++k) {
+        T fk[Q];
+        if (lk & SOLID_BIT) {
+#pragma unroll
+            for (int i = 0; i < Q; ++i) fk[i] = T(0);
+        } else {
+            pull19<T>(h, NP, k, n, b, lk, fk);
+        }
+#pragma unroll
+        for (int i = 0; i < Q; ++i) plane(f, NP, k, i)[n] = fk[i];
+    }
 }
 
 // widen/narrow one [k][i] plane chunk between the context type and the ABI's double
@@ -137,21 +220,25 @@ __global__ void k_links_out(const unsigned* __restrict__ links, unsigned* __rest
 
 // rho^k, u for nodes [n0, n0+cnt) into double staging (Eq. 6-7); solids and empty nodes report 0.
 template <typename T>
-__global__ void k_moments_out(const T* __restrict__ f, long long NP, long long n0, long long cnt,
+__global__ void k_moments_out(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
+                              int nx, int ny, int nz, long long n0, long long cnt,
                               double* __restrict__ o_rr, double* __restrict__ o_rb, double* __restrict__ o_ux,
                               double* __restrict__ o_uy, double* __restrict__ o_uz) {
     const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (t >= cnt) return;
     const long long n = n0 + t;
-    T r[2], jx = T(0), jy = T(0), jz = T(0);
+    const unsigned lk = links ? links[n] : 0u;
+    T r[2] = {T(0), T(0)}, jx = T(0), jy = T(0), jz = T(0);
+    if (!(lk & SOLID_BIT)) {
+        const Nbr b = neighbours(n, nx, ny, nz);
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
-        T fk[Q];
-#pragma unroll
-        for (int i = 0; i < Q; ++i) fk[i] = plane(f, NP, k, i)[n];
-        T ax, ay, az;
-        moments19<T>(fk, r[k], ax, ay, az);
-        jx += ax; jy += ay; jz += az;
+        for (int k = 0; k < 2; ++k) {
+            T fk[Q];
+            pull19<T>(h, NP, k, n, b, lk, fk);
+            T ax, ay, az;
+            moments19<T>(fk, r[k], ax, ay, az);
+            jx += ax; jy += ay; jz += az;
+        }
     }
     const T rt = r[0] + r[1];
     const T inv = rt != T(0) ? T(1) / rt : T(0);
@@ -169,15 +256,18 @@ __device__ __forceinline__ double warp_sum(double v) {
 }
 
 template <typename T>
-__global__ void __launch_bounds__(256) k_diag_partial(const T* __restrict__ f, long long NP, long long N,
-                                                      double* __restrict__ part) {
+__global__ void __launch_bounds__(256) k_diag_partial(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
+                                                      int nx, int ny, int nz, double* __restrict__ part) {
+    const long long N = (long long)nx * ny * nz;
     double acc[5] = {0, 0, 0, 0, 0};
     for (long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x; n < N; n += (long long)gridDim.x * blockDim.x) {
+        const unsigned lk = links ? links[n] : 0u;
+        if (lk & SOLID_BIT) continue;
+        const Nbr b = neighbours(n, nx, ny, nz);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
             T fk[Q];
-#pragma unroll
-            for (int i = 0; i < Q; ++i) fk[i] = plane(f, NP, k, i)[n];
+            pull19<T>(h, NP, k, n, b, lk, fk);
             T r, ax, ay, az;
             moments19<T>(fk, r, ax, ay, az);
             acc[k] += double(r); acc[2] += double(ax); acc[3] += double(ay); acc[4] += double(az);
@@ -218,26 +308,37 @@ __global__ void __launch_bounds__(256) k_diag_final(const double* __restrict__ p
 // ----------------------------------------------------------------------------------------
 // two-pass time step, any box shape
 // ----------------------------------------------------------------------------------------
-// pass 1: rho^k = sum_i f_i^k (Eq. 6).  Solid nodes hold zero populations, so they report 0.
+// pass 1: rho^k(x,t) = sum_i f_i^k(x,t) (Eq. 6) with f pulled from the h-state.  Solid nodes report 0.
+// Also the initialiser of the one-pass kernel's density arrays (rho_in = the whole sum, edge arrays 0).
 template <typename T>
-__global__ void __launch_bounds__(256) k_density(const T* __restrict__ f, long long NP, long long N, T* __restrict__ rho) {
+__global__ void __launch_bounds__(256) k_density(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
+                                                 int nx, int ny, int nz, T* __restrict__ rho) {
+    const long long N = (long long)nx * ny * nz;
     const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (n >= N) return;
+    const unsigned lk = links ? links[n] : 0u;
+    T r[2] = {T(0), T(0)};
+    if (!(lk & SOLID_BIT)) {
+        const Nbr b = neighbours(n, nx, ny, nz);
 #pragma unroll
-    for (int k = 0; k < 2; ++k) {
-        T r = plane(f, NP, k, 0)[n];
-#pragma unroll
-        for (int i = 1; i < Q; ++i) r += plane(f, NP, k, i)[n];
-        rho[(long long)k * NP + n] = r;
+        for (int k = 0; k < 2; ++k) {
+            T fk[Q];
+            pull19<T>(h, NP, k, n, b, lk, fk);
+            T ax, ay, az;
+            moments19<T>(fk, r[k], ax, ay, az);
+        }
     }
+    rho[n] = r[0];
+    rho[NP + n] = r[1];
 }
 
-// pass 2: Shan-Chen force, BGK collision with forcing, bounce-back, periodic streaming (push).
+// pass 2: pull (streaming + bounce-back of the previous step), Shan-Chen force, BGK collision with
+// forcing; the post-collision values are written aligned, to be pulled by the next step.
 template <typename T, bool HAS_SOLID>
-__global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ f, T* __restrict__ g,
-                                                        const T* __restrict__ rho, const unsigned* __restrict__ links,
-                                                        long long NP, int nx, int ny, int nz,
-                                                        T om_r, T om_b, T G) {
+__global__ void __launch_bounds__(256) k_collide_pull(const T* __restrict__ h, T* __restrict__ g,
+                                                      const T* __restrict__ rho, const unsigned* __restrict__ links,
+                                                      long long NP, int nx, int ny, int nz,
+                                                      T om_r, T om_b, T G) {
     const long long N = (long long)nx * ny * nz;
     const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
     if (n >= N) return;
@@ -246,31 +347,23 @@ __global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ f,
         lk = links[n];
         if (lk & SOLID_BIT) return;              // no computation inside a particle
     }
-    const int x = int(n % nx), y = int((n / nx) % ny), z = int(n / ((long long)nx * ny));
-    const int xs[3] = {x == 0 ? nx - 1 : x - 1, x, x == nx - 1 ? 0 : x + 1};
-    const long long ys[3] = {(long long)nx * (y == 0 ? ny - 1 : y - 1), (long long)nx * y, (long long)nx * (y == ny - 1 ? 0 : y + 1)};
-    const long long zs[3] = {(long long)nx * ny * (z == 0 ? nz - 1 : z - 1), (long long)nx * ny * z, (long long)nx * ny * (z == nz - 1 ? 0 : z + 1)};
-    long long nb[Q];
-#pragma unroll
-    for (int i = 0; i < Q; ++i) nb[i] = xs[dir_cx(i) + 1] + ys[dir_cy(i) + 1] + zs[dir_cz(i) + 1];
-
+    const Nbr b = neighbours(n, nx, ny, nz);
     T fr[Q], fb[Q];
-#pragma unroll
-    for (int i = 0; i < Q; ++i) { fr[i] = plane(f, NP, 0, i)[n]; fb[i] = plane(f, NP, 1, i)[n]; }
+    pull19<T>(h, NP, 0, n, b, lk, fr);
+    pull19<T>(h, NP, 1, n, b, lk, fb);
     T rr, rb, jrx, jry, jrz, jbx, jby, jbz;
     moments19<T>(fr, rr, jrx, jry, jrz);
     moments19<T>(fb, rb, jbx, jby, jbz);
-    // the densities this step's force was specified with are pass 1's (index-order sums)
-    rr = rho[n]; rb = rho[NP + n];
     const T den = om_r * rr + om_b * rb;                            // S4
     const T inv = den != T(0) ? T(1) / den : T(0);
     const T ux = (om_r * jrx + om_b * jbx) * inv, uy = (om_r * jry + om_b * jby) * inv, uz = (om_r * jrz + om_b * jbz) * inv;
-    // du^k = -G sum_i w_i rho^kbar(x+c_i) c_i  (S2, S3, S6); solids hold rho = 0 (S7)
+    // du^k = -G sum_i w_i rho^kbar(x+c_i) c_i  (S2, S3, S6); solids report rho = 0 (S7)
     T gr[3] = {T(0), T(0), T(0)}, gb[3] = {T(0), T(0), T(0)};      // gradients of rho_b (acts on red) and rho_r (on blue)
 #pragma unroll
     for (int p = 0; p < 9; ++p) {
-        const T db = w_pair<T>(p) * (rho[NP + nb[2 * p + 1]] - rho[NP + nb[2 * p + 2]]);
-        const T dr = w_pair<T>(p) * (rho[nb[2 * p + 1]] - rho[nb[2 * p + 2]]);
+        const long long np = b.at(pair_cx(p), pair_cy(p), pair_cz(p)), nm = b.at(-pair_cx(p), -pair_cy(p), -pair_cz(p));
+        const T db = w_pair<T>(p) * (rho[NP + np] - rho[NP + nm]);
+        const T dr = w_pair<T>(p) * (rho[np] - rho[nm]);
         if (pair_cx(p)) { gr[0] += T(pair_cx(p)) * db; gb[0] += T(pair_cx(p)) * dr; }
         if (pair_cy(p)) { gr[1] += T(pair_cy(p)) * db; gb[1] += T(pair_cy(p)) * dr; }
         if (pair_cz(p)) { gr[2] += T(pair_cz(p)) * db; gb[2] += T(pair_cz(p)) * dr; }
@@ -279,42 +372,79 @@ __global__ void __launch_bounds__(256) k_collide_stream(const T* __restrict__ f,
     collide19<T>(fb, rb, T(1) - om_b, ux, uy, uz, ux - G * gb[0], uy - G * gb[1], uz - G * gb[2]);
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
-        if (HAS_SOLID && (lk >> i & 1u)) {                          // Eq. 23-24 with u_b = 0
-            plane(g, NP, 0, dir_opp(i))[n] = fr[i];
-            plane(g, NP, 1, dir_opp(i))[n] = fb[i];
-        } else {                                                    // Eq. 5: streaming, periodic
-            plane(g, NP, 0, i)[nb[i]] = fr[i];
-            plane(g, NP, 1, i)[nb[i]] = fb[i];
-        }
+        plane(g, NP, 0, i)[n] = fr[i];
+        plane(g, NP, 1, i)[n] = fb[i];
     }
 }
 
 inline unsigned blocks_for(long long cnt, int bs) { return unsigned((cnt + bs - 1) / bs); }
 
+bool onepass_ok(const lb_ctx* c) { return c->nx % OP_TX == 0 && c->ny % OP_TY == 0; }
+
+// rho_*[rcur] := density of the state in f[cur] (rho_in = the whole sum, the edge arrays zero)
 template <typename T>
-int step_twopass(lb_ctx* c) {
-    const T* f = static_cast<const T*>(c->f[c->cur]);
-    T* g = static_cast<T*>(c->f[c->cur ^ 1]);
-    T* rho = static_cast<T*>(c->rho);
-    const unsigned nb = blocks_for(c->N, 256);
-    k_density<T><<<nb, 256, 0, c->stream>>>(f, c->NP, c->N, rho);
-    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    if (c->has_solid)
-        k_collide_stream<T, true><<<nb, 256, 0, c->stream>>>(f, g, rho, c->links, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
-    else
-        k_collide_stream<T, false><<<nb, 256, 0, c->stream>>>(f, g, rho, nullptr, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
-    c->launches += 2;
+int ensure_rho(lb_ctx* c) {
+    if (c->rho_valid) return LB_OK;
+    const int r = c->rcur;
+    if (c->rho_x[r]) {
+        CU(cudaMemsetAsync(c->rho_x[r], 0, size_t(2) * c->s_x * sizeof(T), c->stream));
+        CU(cudaMemsetAsync(c->rho_y[r], 0, size_t(2) * c->s_y * sizeof(T), c->stream));
+        CU(cudaMemsetAsync(c->rho_xy[r], 0, size_t(2) * c->s_xy * sizeof(T), c->stream));
+    }
+    k_density<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), c->has_solid ? c->links : nullptr,
+                                                               c->NP, c->nx, c->ny, c->nz, static_cast<T*>(c->rho_in[r]));
+    c->launches++;
     CU(cudaGetLastError());
-    c->cur ^= 1;
+    c->rho_valid = true;
     return LB_OK;
 }
 
 template <typename T>
-int zero_solids_both(lb_ctx* c) {
-    for (int b = 0; b < 2; ++b) {
-        k_zero_solids<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<T*>(c->f[b]), c->NP, c->N, c->links);
-        c->launches++;
-    }
+int step_twopass(lb_ctx* c) {
+    c->rho_valid = false;                                   // this path keeps no density across steps
+    const int rc = ensure_rho<T>(c);
+    if (rc != LB_OK) return rc;
+    const T* h = static_cast<const T*>(c->f[c->cur]);
+    T* g = static_cast<T*>(c->f[c->cur ^ 1]);
+    const T* rho = static_cast<const T*>(c->rho_in[c->rcur]);
+    const unsigned nb = blocks_for(c->N, 256);
+    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
+    if (c->has_solid)
+        k_collide_pull<T, true><<<nb, 256, 0, c->stream>>>(h, g, rho, c->links, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
+    else
+        k_collide_pull<T, false><<<nb, 256, 0, c->stream>>>(h, g, rho, nullptr, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    c->cur ^= 1;
+    c->rho_valid = false;
+    return LB_OK;
+}
+
+template <typename T>
+int zero_solids(lb_ctx* c, int buf) {
+    k_zero_solids<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<T*>(c->f[buf]), c->NP, c->N, c->links);
+    c->launches++;
+    CU(cudaGetLastError());
+    return LB_OK;
+}
+
+// f in the scratch buffer -> h-state in f[cur]; the scratch keeps zeros on solid nodes
+template <typename T>
+int unstream_scratch(lb_ctx* c) {
+    k_unstream<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur ^ 1]), static_cast<T*>(c->f[c->cur]),
+                                                                c->has_solid ? c->links : nullptr, c->NP, c->nx, c->ny, c->nz);
+    c->launches++;
+    CU(cudaGetLastError());
+    c->rho_valid = false;
+    return LB_OK;
+}
+
+// h-state -> f in the scratch buffer
+template <typename T>
+int stream_to_scratch(lb_ctx* c) {
+    k_stream<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), static_cast<T*>(c->f[c->cur ^ 1]),
+                                                              c->has_solid ? c->links : nullptr, c->NP, c->nx, c->ny, c->nz);
+    c->launches++;
     CU(cudaGetLastError());
     return LB_OK;
 }
@@ -322,19 +452,16 @@ int zero_solids_both(lb_ctx* c) {
 // ----------------------------------------------------------------------------------------
 // one-pass time step (lb_onepass.cuh): boxes whose x, y sides are multiples of the 32 x 8 tile
 // ----------------------------------------------------------------------------------------
-constexpr int OP_TX = 32, OP_TY = 8;
 constexpr int OP_RESIDENT_CTAS = 148 * 2;
 
-bool onepass_ok(const lb_ctx* c) { return c->nx % OP_TX == 0 && c->ny % OP_TY == 0; }
-
-// planes per CTA: long enough to amortise the 2-plane density prologue, short enough that the
-// grid is many waves of the resident CTAs; a divisor of nz when one is close.
+// planes per CTA: every chunk re-collides 2 extra planes, so long chunks; but the grid should
+// still be several waves of the resident CTAs.  LB_ONEPASS_ZC overrides (tuning).
 int onepass_zc(const lb_ctx* c) {
     if (const char* e = std::getenv("LB_ONEPASS_ZC")) { const int v = std::atoi(e); if (v >= 1) return v < c->nz ? v : c->nz; }
     const long long tiles = (long long)(c->nx / OP_TX) * (c->ny / OP_TY);
-    const long long chunks_wanted = (OP_RESIDENT_CTAS * 6 + tiles - 1) / tiles;
+    const long long chunks_wanted = (OP_RESIDENT_CTAS * 4 + tiles - 1) / (tiles > 0 ? tiles : 1);
     long long zc = c->nz / (chunks_wanted > 0 ? chunks_wanted : 1);
-    if (zc > 64) zc = 64;
+    if (zc > 128) zc = 128;
     if (zc < 16) zc = 16;
     if (zc > c->nz) zc = c->nz;
     for (long long d = zc; d >= (zc + 1) / 2; --d)
@@ -343,19 +470,42 @@ int onepass_zc(const lb_ctx* c) {
 }
 
 template <typename T>
-int step_onepass(lb_ctx* c) {
-    const T* f = static_cast<const T*>(c->f[c->cur]);
-    T* g = static_cast<T*>(c->f[c->cur ^ 1]);
-    const int zc = onepass_zc(c);
-    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + zc - 1) / zc);
+RhoView<T> rho_view(const lb_ctx* c, int r) {
+    RhoView<T> v;
+    v.in = static_cast<T*>(c->rho_in[r]); v.s_in = c->NP;
+    v.x = static_cast<T*>(c->rho_x[r]); v.s_x = c->s_x;
+    v.y = static_cast<T*>(c->rho_y[r]); v.s_y = c->s_y;
+    v.xy = static_cast<T*>(c->rho_xy[r]); v.s_xy = c->s_xy;
+    return v;
+}
+
+template <typename T, bool HAS_SOLID>
+int launch_onepass(lb_ctx* c) {
+    auto kern = k_step_pull<T, HAS_SOLID, OP_TX, OP_TY>;
+    constexpr size_t smem = onepass_smem_bytes<T, OP_TX, OP_TY>();
+    static bool configured = false;                         // per instantiation
+    if (!configured) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
+        configured = true;
+    }
+    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc - 1) / c->zc);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    if (c->has_solid)
-        k_step_onepass<T, true, OP_TX, OP_TY><<<grid, OP_TX * OP_TY, 0, c->stream>>>(f, g, c->links, c->NP, c->nx, c->ny, c->nz, zc, om_r, om_b, G);
-    else
-        k_step_onepass<T, false, OP_TX, OP_TY><<<grid, OP_TX * OP_TY, 0, c->stream>>>(f, g, nullptr, c->NP, c->nx, c->ny, c->nz, zc, om_r, om_b, G);
+    kern<<<grid, OP_TX * OP_TY, smem, c->stream>>>(static_cast<const T*>(c->f[c->cur]), static_cast<T*>(c->f[c->cur ^ 1]),
+                                                   HAS_SOLID ? c->links : nullptr, rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1),
+                                                   c->NP, c->nx, c->ny, c->nz, c->zc, om_r, om_b, G);
     c->launches += 1;
     CU(cudaGetLastError());
+    return LB_OK;
+}
+
+template <typename T>
+int step_onepass(lb_ctx* c) {
+    int rc = ensure_rho<T>(c);
+    if (rc != LB_OK) return rc;
+    rc = c->has_solid ? launch_onepass<T, true>(c) : launch_onepass<T, false>(c);
+    if (rc != LB_OK) return rc;
     c->cur ^= 1;
+    c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
     return LB_OK;
 }
 
@@ -365,6 +515,8 @@ int resolve_kernel(lb_ctx* c, int kind) {
     return kind;
 }
 
+long long round64(long long v) { return (v + 63) / 64 * 64; }
+
 }  // namespace
 
 // ----------------------------------------------------------------------------------------
@@ -373,7 +525,7 @@ int resolve_kernel(lb_ctx* c, int kind) {
 extern "C" {
 
 const char* lb_last_error(void) { return g_err.c_str(); }
-const char* lb_version(void) { return "lb-b200 0.1 (sm_100a)"; }
+const char* lb_version(void) { return "lb-b200 0.2 (sm_100a)"; }
 
 lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double G, int dtype, void* cuda_stream) {
     g_err.clear();
@@ -395,7 +547,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     std::memset(c, 0, sizeof(*c));
     c->nx = nx; c->ny = ny; c->nz = nz;
     c->N = (long long)nx * ny * nz;
-    c->NP = (c->N + 63) / 64 * 64;
+    c->NP = round64(c->N);
     c->dtype = dtype;
     c->tau[0] = tau_r; c->tau[1] = tau_b; c->G = G;
     if (cuda_stream) { c->stream = static_cast<cudaStream_t>(cuda_stream); c->own_stream = false; }
@@ -409,7 +561,18 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     bool ok = true;
     ok = ok && cudaMalloc(&c->f[0], fbytes) == cudaSuccess;
     ok = ok && cudaMalloc(&c->f[1], fbytes) == cudaSuccess;
-    ok = ok && cudaMalloc(&c->rho, size_t(2) * c->NP * es) == cudaSuccess;
+    for (int r = 0; r < 2; ++r) ok = ok && cudaMalloc(&c->rho_in[r], size_t(2) * c->NP * es) == cudaSuccess;
+    if (onepass_ok(c)) {
+        const long long ntx = nx / OP_TX, nty = ny / OP_TY;
+        c->s_x = round64((long long)nz * nty * ntx * 2 * OP_TY);
+        c->s_y = round64((long long)nz * nty * 2 * nx);
+        c->s_xy = round64((long long)nz * nty * ntx * 4);
+        for (int r = 0; r < 2; ++r) {
+            ok = ok && cudaMalloc(&c->rho_x[r], size_t(2) * c->s_x * es) == cudaSuccess;
+            ok = ok && cudaMalloc(&c->rho_y[r], size_t(2) * c->s_y * es) == cudaSuccess;
+            ok = ok && cudaMalloc(&c->rho_xy[r], size_t(2) * c->s_xy * es) == cudaSuccess;
+        }
+    }
     ok = ok && cudaMalloc(&c->links, size_t(c->N) * sizeof(unsigned)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->stage, size_t(STAGE_NODES) * 5 * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->diag_part, size_t(DIAG_BLOCKS) * 5 * sizeof(double)) == cudaSuccess;
@@ -417,7 +580,6 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     if (ok) {
         ok = ok && cudaMemsetAsync(c->f[0], 0, fbytes, c->stream) == cudaSuccess;
         ok = ok && cudaMemsetAsync(c->f[1], 0, fbytes, c->stream) == cudaSuccess;
-        ok = ok && cudaMemsetAsync(c->rho, 0, size_t(2) * c->NP * es, c->stream) == cudaSuccess;
         ok = ok && cudaMemsetAsync(c->links, 0, size_t(c->N) * sizeof(unsigned), c->stream) == cudaSuccess;
     }
     if (!ok) {
@@ -428,6 +590,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     }
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
+    c->zc = onepass_zc(c);
     return c;
 }
 
@@ -438,7 +601,8 @@ lb_ctx* lb_create(int nx, int ny, int nz, double tau_r, double tau_b, double G) 
 void lb_destroy(lb_ctx* c) {
     if (!c) return;
     cudaStreamSynchronize(c->stream);
-    cudaFree(c->f[0]); cudaFree(c->f[1]); cudaFree(c->rho); cudaFree(c->links);
+    cudaFree(c->f[0]); cudaFree(c->f[1]); cudaFree(c->links);
+    for (int r = 0; r < 2; ++r) { cudaFree(c->rho_in[r]); cudaFree(c->rho_x[r]); cudaFree(c->rho_y[r]); cudaFree(c->rho_xy[r]); }
     cudaFree(c->stage); cudaFree(c->diag_part); cudaFree(c->diag_out);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
@@ -464,6 +628,13 @@ int lb_set_kernel(lb_ctx* c, int kind) {
 
 int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
     if (!c || !mask) return fail(LB_EINVAL, "NULL argument");
+    const bool f64 = c->dtype == LB_F64;
+    int rc;
+    // the fields already set are defined on nodes (f): take them out of the h-state under the OLD links
+    if (c->have_fields) {
+        rc = f64 ? stream_to_scratch<double>(c) : stream_to_scratch<float>(c);
+        if (rc != LB_OK) return rc;
+    }
     unsigned char* d_mask = nullptr;
     CU(cudaMalloc(&d_mask, size_t(c->N)));
     cudaError_t e = cudaMemcpyAsync(d_mask, mask, size_t(c->N), cudaMemcpyHostToDevice, c->stream);
@@ -476,7 +647,12 @@ int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
     cudaFree(d_mask);
     if (e != cudaSuccess) return fail_cuda(e, "lb_set_solid_mask");
     c->has_solid = true;   // a mask of all zeros still takes the (slower) link-checking kernels
-    return c->dtype == LB_F64 ? zero_solids_both<double>(c) : zero_solids_both<float>(c);
+    c->rho_valid = false;
+    // S8: solid nodes hold exactly 0 in both buffers (the step kernels never write them)
+    rc = f64 ? zero_solids<double>(c, c->cur ^ 1) : zero_solids<float>(c, c->cur ^ 1);
+    if (rc != LB_OK) return rc;
+    if (c->have_fields) return f64 ? unstream_scratch<double>(c) : unstream_scratch<float>(c);
+    return f64 ? zero_solids<double>(c, c->cur) : zero_solids<float>(c, c->cur);
 }
 
 int lb_set_fields(lb_ctx* c, const double* rho_r, const double* rho_b, const double* ux, const double* uy, const double* uz) {
@@ -484,6 +660,7 @@ int lb_set_fields(lb_ctx* c, const double* rho_r, const double* rho_b, const dou
     const int nu = (ux != nullptr) + (uy != nullptr) + (uz != nullptr);
     if (nu != 0 && nu != 3) return fail(LB_EINVAL, "ux, uy, uz must be all NULL or all non-NULL");
     const double* src[5] = {rho_r, rho_b, ux, uy, uz};
+    void* scratch = c->f[c->cur ^ 1];
     for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES) {
         const long long cnt = (c->N - n0 < STAGE_NODES) ? c->N - n0 : STAGE_NODES;
         double* st[5];
@@ -493,12 +670,14 @@ int lb_set_fields(lb_ctx* c, const double* rho_r, const double* rho_b, const dou
         }
         const unsigned* lk = c->has_solid ? c->links : nullptr;
         if (c->dtype == LB_F64)
-            k_init_eq<double><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<double*>(c->f[c->cur]), c->NP, n0, cnt, st[0], st[1], st[2], st[3], st[4], lk);
+            k_init_eq<double><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<double*>(scratch), c->NP, n0, cnt, st[0], st[1], st[2], st[3], st[4], lk);
         else
-            k_init_eq<float><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<float*>(c->f[c->cur]), c->NP, n0, cnt, st[0], st[1], st[2], st[3], st[4], lk);
+            k_init_eq<float><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<float*>(scratch), c->NP, n0, cnt, st[0], st[1], st[2], st[3], st[4], lk);
         c->launches++;
         CU(cudaGetLastError());
     }
+    const int rc = c->dtype == LB_F64 ? unstream_scratch<double>(c) : unstream_scratch<float>(c);
+    if (rc != LB_OK) return rc;
     CU(cudaStreamSynchronize(c->stream));          // the caller's arrays are free again
     c->have_fields = true;
     return LB_OK;
@@ -506,12 +685,13 @@ int lb_set_fields(lb_ctx* c, const double* rho_r, const double* rho_b, const dou
 
 int lb_set_populations(lb_ctx* c, const double* f) {
     if (!c || !f) return fail(LB_EINVAL, "NULL argument");
+    void* scratch = c->f[c->cur ^ 1];
     for (int q = 0; q < NPOP; ++q) {
         const double* src = f + (long long)q * c->N;
         if (c->dtype == LB_F64) {
-            CU(cudaMemcpyAsync(static_cast<double*>(c->f[c->cur]) + (long long)q * c->NP, src, size_t(c->N) * 8, cudaMemcpyHostToDevice, c->stream));
+            CU(cudaMemcpyAsync(static_cast<double*>(scratch) + (long long)q * c->NP, src, size_t(c->N) * 8, cudaMemcpyHostToDevice, c->stream));
         } else {
-            float* dst = static_cast<float*>(c->f[c->cur]) + (long long)q * c->NP;
+            float* dst = static_cast<float*>(scratch) + (long long)q * c->NP;
             for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES * 5) {
                 const long long cnt = (c->N - n0 < STAGE_NODES * 5) ? c->N - n0 : STAGE_NODES * 5;
                 CU(cudaMemcpyAsync(c->stage, src + n0, size_t(cnt) * 8, cudaMemcpyHostToDevice, c->stream));
@@ -521,10 +701,13 @@ int lb_set_populations(lb_ctx* c, const double* f) {
             }
         }
     }
+    int rc;
     if (c->has_solid) {
-        const int rc = c->dtype == LB_F64 ? zero_solids_both<double>(c) : zero_solids_both<float>(c);
+        rc = c->dtype == LB_F64 ? zero_solids<double>(c, c->cur ^ 1) : zero_solids<float>(c, c->cur ^ 1);
         if (rc != LB_OK) return rc;
     }
+    rc = c->dtype == LB_F64 ? unstream_scratch<double>(c) : unstream_scratch<float>(c);
+    if (rc != LB_OK) return rc;
     CU(cudaStreamSynchronize(c->stream));
     c->have_fields = true;
     return LB_OK;
@@ -545,12 +728,15 @@ int lb_step(lb_ctx* c, int nsteps) {
 
 int lb_get_populations(lb_ctx* c, double* f) {
     if (!c || !f) return fail(LB_EINVAL, "NULL argument");
+    const int rc = c->dtype == LB_F64 ? stream_to_scratch<double>(c) : stream_to_scratch<float>(c);
+    if (rc != LB_OK) return rc;
+    const void* scratch = c->f[c->cur ^ 1];
     for (int q = 0; q < NPOP; ++q) {
         double* dst = f + (long long)q * c->N;
         if (c->dtype == LB_F64) {
-            CU(cudaMemcpyAsync(dst, static_cast<const double*>(c->f[c->cur]) + (long long)q * c->NP, size_t(c->N) * 8, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaMemcpyAsync(dst, static_cast<const double*>(scratch) + (long long)q * c->NP, size_t(c->N) * 8, cudaMemcpyDeviceToHost, c->stream));
         } else {
-            const float* src = static_cast<const float*>(c->f[c->cur]) + (long long)q * c->NP;
+            const float* src = static_cast<const float*>(scratch) + (long long)q * c->NP;
             for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES * 5) {
                 const long long cnt = (c->N - n0 < STAGE_NODES * 5) ? c->N - n0 : STAGE_NODES * 5;
                 k_to_double<float><<<blocks_for(cnt, 256), 256, 0, c->stream>>>(src + n0, c->stage, cnt);
@@ -567,14 +753,15 @@ int lb_get_populations(lb_ctx* c, double* f) {
 int lb_get_moments(lb_ctx* c, double* rho_r, double* rho_b, double* ux, double* uy, double* uz) {
     if (!c) return fail(LB_EINVAL, "NULL context");
     double* dst[5] = {rho_r, rho_b, ux, uy, uz};
+    const unsigned* lk = c->has_solid ? c->links : nullptr;
     for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES) {
         const long long cnt = (c->N - n0 < STAGE_NODES) ? c->N - n0 : STAGE_NODES;
         double* st[5];
         for (int a = 0; a < 5; ++a) st[a] = c->stage + a * STAGE_NODES;
         if (c->dtype == LB_F64)
-            k_moments_out<double><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), c->NP, n0, cnt, st[0], st[1], st[2], st[3], st[4]);
+            k_moments_out<double><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, n0, cnt, st[0], st[1], st[2], st[3], st[4]);
         else
-            k_moments_out<float><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<const float*>(c->f[c->cur]), c->NP, n0, cnt, st[0], st[1], st[2], st[3], st[4]);
+            k_moments_out<float><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<const float*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, n0, cnt, st[0], st[1], st[2], st[3], st[4]);
         c->launches++;
         CU(cudaGetLastError());
         for (int a = 0; a < 5; ++a)
@@ -601,10 +788,11 @@ int lb_get_link_mask(lb_ctx* c, unsigned int* links) {
 
 int lb_get_diagnostics(lb_ctx* c, double mass[2], double momentum[3]) {
     if (!c || !mass || !momentum) return fail(LB_EINVAL, "NULL argument");
+    const unsigned* lk = c->has_solid ? c->links : nullptr;
     if (c->dtype == LB_F64)
-        k_diag_partial<double><<<DIAG_BLOCKS, 256, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), c->NP, c->N, c->diag_part);
+        k_diag_partial<double><<<DIAG_BLOCKS, 256, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, c->diag_part);
     else
-        k_diag_partial<float><<<DIAG_BLOCKS, 256, 0, c->stream>>>(static_cast<const float*>(c->f[c->cur]), c->NP, c->N, c->diag_part);
+        k_diag_partial<float><<<DIAG_BLOCKS, 256, 0, c->stream>>>(static_cast<const float*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, c->diag_part);
     k_diag_final<<<1, 256, 0, c->stream>>>(c->diag_part, DIAG_BLOCKS, c->diag_out);
     c->launches += 2;
     CU(cudaGetLastError());
