@@ -15,23 +15,30 @@
 //   Recomputing the neighbours' densities costs either a second sweep (944 B/node) or, per tile,
 //   halo reads that miss in L2 (measured: 824 B/node of DRAM traffic).  Instead step t produces
 //   rho(.,t+1) itself: rho(y,t+1) = sum_i h_i(y - c_i), a gather over the post-collision values
-//   the CTA has just computed.  One CTA owns a TX x TY column and marches along z:
-//     - post-collision values are exchanged through shared memory (16 direction planes S_i,
-//       zero-padded by two nodes), each thread gathers the three in-plane partial sums
-//       A_dz = sum_{i: cz_i = dz} h_i(y - c_i) of its node and pipelines them along z in
-//       registers: rho(z) = (A_+1(z-1) + A_0(z)) + A_-1(z+1);
-//     - contributions that cross a tile edge are NOT added into the neighbour's array (that
-//       would need atomics and give an order-dependent fp sum).  Each of the four arrays
-//       rho_in / rho_x / rho_y / rho_xy has exactly ONE writer per entry: the owner tile (in),
-//       its x neighbour (x), its y neighbour (y), its diagonal neighbour (xy).  The reader
-//       assembles rho = ((in + x) + y) + xy in that fixed order: deterministic, and every CTA
-//       that needs a node's density computes the same bits;
-//     - along z the chunk [z0,z1) re-collides planes z0-1 and z1 (without storing them) so
-//       that no partial sums cross chunk boundaries: 2/zc extra reads.
-//   rho(t) for the tile and its one-node halo lives in a shared-memory ring of four planes.
-//   u' needs j of BOTH components before either is collided (S4): the blue populations are
-//   pulled once for their moments, then again (L1/L2 hits) for their collision, so that only
-//   19 values are live at a time (<= 128 registers, two 256-thread CTAs per SM).
+//   the CTA has just computed.  One CTA owns a 32 x TY column (one warp per row) and marches
+//   along z.  The gather is separable:
+//     x:  row sums  U0/Up/Um[dz] = h(x) + h(x-1) + h(x+1)  over the directions with cy = 0/+1/-1,
+//         cz = dz, by warp shuffles;
+//     y:  A_dz(y) = U0[dz](y) + Up[dz](y-1) + Um[dz](y+1)  through shared memory (6 planes per
+//         component);
+//     z:  rho(z) = (A_+1(z-1) + A_0(z)) + A_-1(z+1)  pipelined in registers.
+//   Contributions that cross a tile edge are NOT added into the neighbour's array (that would
+//   need atomics and give an order-dependent fp sum).  Each of the four arrays rho_in / rho_x /
+//   rho_y / rho_xy has exactly ONE writer per entry: the owner tile (in), its x neighbour (x),
+//   its y neighbour (y), its diagonal neighbour (xy).  The reader assembles
+//   rho = ((in + x) + y) + xy in that fixed order: deterministic, and every CTA that needs a
+//   node's density computes the same bits.  Along z the chunk [z0,z1) re-collides planes z0-1
+//   and z1 (without storing them) so that no partial sums cross chunk boundaries: 2/zc extra
+//   reads.  rho(t) for the tile and its one-node halo lives in a shared-memory ring of four planes,
+//   filled two planes ahead with cp.async.
+//
+// Latency hiding (two 256-thread CTAs per SM, <= 128 registers, two barriers per plane):
+//   u' needs j of BOTH components before either is collided (S4), and 38 live populations do
+//   not fit the register budget.  The blue populations of the NEXT plane are therefore pulled
+//   with cp.async into a thread-private shared-memory stash (no registers in flight, no barrier:
+//   a thread only reads its own slots); their moments and their collision stream out of the
+//   stash pair by pair.  The red populations of the next plane are pulled into the one register
+//   array as soon as this plane's red collision has been published.
 #pragma once
 #include "lb_lattice.cuh"
 
@@ -45,31 +52,57 @@ struct RhoView {
     T* in;  long long s_in;     // [k][NP]                              node n
     T* x;   long long s_x;      // [k][z][tile_y][tile_x][side][TY]     nodes with x_local in {0, TX-1}
     T* y;   long long s_y;      // [k][z][tile_y][side][nx]             nodes with y_local in {0, TY-1}
-    T* xy;  long long s_xy;     // [k][z][tile_y][tile_x][4]            tile corners
+    T* xy;  long long s_xy;     // [k][z][tile_y][tile_x][4]            tile corners, index 2*(y_local != 0) + (x_local != 0)
 };
 
-// index of direction i in the shared exchange planes (directions with an in-plane offset)
-__host__ __device__ constexpr int sidx(int i) { return i <= 4 ? i - 1 : i - 3; }
-__host__ __device__ constexpr bool dir_local(int i) { return dir_cx(i) == 0 && dir_cy(i) == 0; }
+template <int TX, int TY>
+struct OnepassLayout {
+    static constexpr int NT = TX * TY;
+    static constexpr int RW = TX + 2, RH = TY + 2, RS = RW * RH;       // tile + one-node frame
+    static constexpr int NPX = 4 * RH, NPY = 4 * RW, NPXY = 16, NPIECE = NPX + NPY + NPXY;
+    static constexpr int NEDGE = NPX + 4 * (RW - 4);                   // ring positions that have edge pieces
+    // element offsets into shared memory
+    static constexpr int RING = 0;                                     // [4][2][RS]   rho(t), planes z-1..z+2
+    static constexpr int SU = RING + 8 * RS;                           // [2][6][RS]   Up[dz], Um[dz] per component; frame = 0
+    static constexpr int STASH = SU + 12 * RS;                         // [Q][NT]      pulled blue populations of this thread
+    static constexpr int STAGE = STASH + Q * NT;                       // [2][NPIECE]  edge pieces of the ring plane being filled
+    static constexpr int E0 = STAGE + 2 * NPIECE;                      // [2][3][2][TY] U0[dz] of the virtual columns -1 and TX
+    static constexpr int ACCR = E0 + 12 * TY;                          // [2][2][TX][2] z pipelines of the row exports
+    static constexpr int ACCC = ACCR + 8 * TX;                         // [2][2][TY][2] z pipelines of the column exports
+    static constexpr int TOTAL = ACCC + 8 * TY;
+};
 
 template <typename T, int TX, int TY>
-constexpr size_t onepass_smem_bytes() {
-    return sizeof(T) * (size_t(8) * (TX + 2) * (TY + 2) + size_t(16) * (TX + 4) * (TY + 4));
+constexpr size_t onepass_smem_bytes() { return sizeof(T) * size_t(OnepassLayout<TX, TY>::TOTAL); }
+
+template <int BYTES>
+__device__ __forceinline__ void cp_async(void* smem_dst, const void* gsrc) {
+    const unsigned d = static_cast<unsigned>(__cvta_generic_to_shared(smem_dst));
+    asm volatile("cp.async.ca.shared.global [%0], [%1], %2;\n" ::"r"(d), "l"(gsrc), "n"(BYTES) : "memory");
 }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory"); }
 
 template <typename T, bool HAS_SOLID, int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, 2)
 k_step_pull(const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
             const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
             T om_r, T om_b, T G) {
-    constexpr int NT = TX * TY;
-    constexpr int RW = TX + 2, RH = TY + 2, RS = RW * RH;      // density ring plane: tile + 1 halo
-    constexpr int PW = TX + 4, PH = TY + 4, PS = PW * PH;      // exchange plane: tile + 2 zero padding
-    constexpr int NHALO = 2 * RW + 2 * TY;
-    static_assert(NHALO <= NT, "one halo node per thread at most");
+    using L = OnepassLayout<TX, TY>;
+    static_assert(TX == 32, "one warp per tile row: the x gather uses warp shuffles");
+    constexpr int NT = L::NT, RW = L::RW, RH = L::RH, RS = L::RS;
+    constexpr int NPX = L::NPX, NPY = L::NPY, NPIECE = L::NPIECE, NEDGE = L::NEDGE;
+    static_assert(NPIECE <= NT && NEDGE <= NT && RS <= 2 * NT, "ring fill work must fit the CTA");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    T* ring = reinterpret_cast<T*>(smem_raw);                  // [4][2][RS]
-    T* S = ring + 8 * RS;                                      // [16][PS]
+    T* sm = reinterpret_cast<T*>(smem_raw);
+    T* ring = sm + L::RING;
+    T* SU = sm + L::SU;
+    T* stash = sm + L::STASH;
+    T* stage = sm + L::STAGE;
+    T* e0a = sm + L::E0;
+    T* accr = sm + L::ACCR;
+    T* accc = sm + L::ACCC;
 
     const int t = threadIdx.x;
     const int tx = t % TX, ty = t / TX;
@@ -80,169 +113,240 @@ k_step_pull(const T* __restrict__ h, T* __restrict__ g, const unsigned* __restri
     const int z1 = min(z0 + zc, nz);
     const long long pl = (long long)nx * ny;
     const long long psx = (long long)nty * ntx * 2 * TY, psy = (long long)nty * 2 * nx, psxy = (long long)nty * ntx * 4;
+    const int btxm = btx == 0 ? ntx - 1 : btx - 1, btxp = btx == ntx - 1 ? 0 : btx + 1;
+    const int btym = bty == 0 ? nty - 1 : bty - 1, btyp = bty == nty - 1 ? 0 : bty + 1;
 
-    for (int a = t; a < 16 * PS; a += NT) S[a] = T(0);         // padding stays zero for the whole kernel
+    for (int a = t; a < L::STASH - L::SU; a += NT) SU[a] = T(0);          // the frame stays zero for the whole kernel
+    for (int a = t; a < L::TOTAL - L::STAGE; a += NT) stage[a] = T(0);   // stage, e0, export pipelines
 
     // periodic neighbours in x and y (element offsets within a plane)
     const int xs[3] = {x == 0 ? nx - 1 : x - 1, x, x == nx - 1 ? 0 : x + 1};
     const int ys[3] = {nx * (y == 0 ? ny - 1 : y - 1), nx * y, nx * (y == ny - 1 ? 0 : y + 1)};
     const int own_xy = ys[1] + x;
     const int own_r = (ty + 1) * RW + tx + 1;
-    const int own_p = (ty + 2) * PW + tx + 2;
-    const bool own_ex = (tx == 0 || tx == TX - 1), own_ey = (ty == 0 || ty == TY - 1);
-    const int own_ox = ((bty * ntx + btx) * 2 + (tx != 0)) * TY + ty;
-    const int own_oy = (bty * 2 + (ty != 0)) * nx + x;
-    const int own_oxy = (bty * ntx + btx) * 4 + (ty != 0) * 2 + (tx != 0);
-
-    // the halo node this thread assembles (ring) and exports to (tile-relative hx in [-1,TX], hy in [-1,TY])
-    const bool has_halo = t < NHALO;
-    int halo_in = 0, halo_r = 0, halo_p = 0, halo_ox = 0, halo_oy = 0, halo_oxy = 0;
-    bool halo_ex = false, halo_ey = false;
-    if (has_halo) {
-        int hx, hy;
-        if (t < RW) { hx = t - 1; hy = -1; }
-        else if (t < 2 * RW) { hx = t - RW - 1; hy = TY; }
-        else if (t < 2 * RW + TY) { hx = -1; hy = t - 2 * RW; }
-        else { hx = TX; hy = t - 2 * RW - TY; }
-        const int otx = hx < 0 ? (btx == 0 ? ntx - 1 : btx - 1) : (hx >= TX ? (btx == ntx - 1 ? 0 : btx + 1) : btx);
-        const int oty = hy < 0 ? (bty == 0 ? nty - 1 : bty - 1) : (hy >= TY ? (bty == nty - 1 ? 0 : bty + 1) : bty);
-        const int lx = hx < 0 ? TX - 1 : (hx >= TX ? 0 : hx);
-        const int ly = hy < 0 ? TY - 1 : (hy >= TY ? 0 : hy);
-        const int gx = otx * TX + lx, gy = oty * TY + ly;
-        halo_in = gy * nx + gx;
-        halo_r = (hy + 1) * RW + hx + 1;
-        halo_p = (hy + 2) * PW + hx + 2;
-        halo_ex = (lx == 0 || lx == TX - 1);
-        halo_ey = (ly == 0 || ly == TY - 1);
-        halo_ox = ((oty * ntx + otx) * 2 + (lx != 0)) * TY + ly;
-        halo_oy = (oty * 2 + (ly != 0)) * nx + gx;
-        halo_oxy = (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
-    }
-    // which single-writer array this CTA's contribution to its halo node goes to
-    const bool halo_col = has_halo && t >= 2 * RW;                                    // hx outside, hy inside
-    const bool halo_corner = has_halo && t < 2 * RW && (t % RW == 0 || t % RW == RW - 1);
 
     auto wrapz = [&](int p) { p %= nz; return p < 0 ? p + nz : p; };
 
-    // rho(t) of plane p at the own node and at the halo node: ((in + x) + y) + xy
-    auto ring_load = [&](int p, T (&v)[4]) {
-        const long long zl = wrapz(p);
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            T a = __ldg(ri.in + k * ri.s_in + zl * pl + own_xy);
-            if (own_ex) a += __ldg(ri.x + k * ri.s_x + zl * psx + own_ox);
-            if (own_ey) a += __ldg(ri.y + k * ri.s_y + zl * psy + own_oy);
-            if (own_ex && own_ey) a += __ldg(ri.xy + k * ri.s_xy + zl * psxy + own_oxy);
-            v[k] = a;
-            if (has_halo) {
-                T b = __ldg(ri.in + k * ri.s_in + zl * pl + halo_in);
-                if (halo_ex) b += __ldg(ri.x + k * ri.s_x + zl * psx + halo_ox);
-                if (halo_ey) b += __ldg(ri.y + k * ri.s_y + zl * psy + halo_oy);
-                if (halo_ex && halo_ey) b += __ldg(ri.xy + k * ri.s_xy + zl * psxy + halo_oxy);
-                v[2 + k] = b;
-            }
-        }
+    // ---- ring fill: what this thread copies for every plane ------------------------------------
+    // tile-relative (rx, ry) in [-1,TX] x [-1,TY] -> owner tile, local coordinates, global x / y
+    auto owner = [&](int rx, int ry, int& otx, int& oty, int& lx, int& ly) {
+        otx = rx < 0 ? btxm : (rx >= TX ? btxp : btx);
+        oty = ry < 0 ? btym : (ry >= TY ? btyp : bty);
+        lx = rx < 0 ? TX - 1 : (rx >= TX ? 0 : rx);
+        ly = ry < 0 ? TY - 1 : (ry >= TY ? 0 : ry);
     };
-    auto ring_store = [&](int p, const T (&v)[4]) {
+    int in_off[2] = {0, -1};                                             // rho_in offsets of ring positions t, t + NT
+#pragma unroll
+    for (int a = 0; a < 2; ++a) {
+        const int pos = t + a * NT;
+        if (pos < RS) {
+            int otx, oty, lx, ly;
+            owner(pos % RW - 1, pos / RW - 1, otx, oty, lx, ly);
+            in_off[a] = (oty * TY + ly) * nx + otx * TX + lx;
+        }
+    }
+    int piece_off = -1, piece_kind = 0;                                  // edge piece t: 0 = x, 1 = y, 2 = xy
+    if (t < NPIECE) {
+        int rx, ry;
+        if (t < NPX) { const int c4 = t / RH; rx = c4 == 0 ? -1 : (c4 == 1 ? 0 : (c4 == 2 ? TX - 1 : TX)); ry = t % RH - 1; piece_kind = 0; }
+        else if (t < NPX + NPY) { const int q = t - NPX, r4 = q / RW; ry = r4 == 0 ? -1 : (r4 == 1 ? 0 : (r4 == 2 ? TY - 1 : TY)); rx = q % RW - 1; piece_kind = 1; }
+        else { const int q = t - NPX - NPY, r4 = q / 4, c4 = q % 4;
+               ry = r4 == 0 ? -1 : (r4 == 1 ? 0 : (r4 == 2 ? TY - 1 : TY)); rx = c4 == 0 ? -1 : (c4 == 1 ? 0 : (c4 == 2 ? TX - 1 : TX)); piece_kind = 2; }
+        int otx, oty, lx, ly;
+        owner(rx, ry, otx, oty, lx, ly);
+        if (piece_kind == 0) piece_off = ((oty * ntx + otx) * 2 + (lx != 0)) * TY + ly;
+        else if (piece_kind == 1) piece_off = (oty * 2 + (ly != 0)) * nx + otx * TX + lx;
+        else piece_off = (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
+    }
+    // rho(t) of plane p: the rho_in part goes straight into the ring, the edge pieces into `stage`
+    auto ring_issue = [&](int p) {
+        const long long zl = wrapz(p);
         const int slot = (p - z0 + 2) & 3;
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
-            ring[(slot * 2 + k) * RS + own_r] = v[k];
-            if (has_halo) ring[(slot * 2 + k) * RS + halo_r] = v[2 + k];
+            T* dst = ring + (slot * 2 + k) * RS;
+            cp_async<sizeof(T)>(dst + t, ri.in + k * ri.s_in + zl * pl + in_off[0]);
+            if (in_off[1] >= 0) cp_async<sizeof(T)>(dst + t + NT, ri.in + k * ri.s_in + zl * pl + in_off[1]);
+            if (piece_off >= 0) {
+                const T* src = piece_kind == 0 ? ri.x + k * ri.s_x + zl * psx
+                             : (piece_kind == 1 ? ri.y + k * ri.s_y + zl * psy : ri.xy + k * ri.s_xy + zl * psxy);
+                cp_async<sizeof(T)>(stage + k * NPIECE + t, src + piece_off);
+            }
+        }
+        cp_async_commit();
+    };
+    // rho = ((in + x) + y) + xy on the ring positions that have edge pieces (after a barrier)
+    auto ring_assemble = [&](int p) {
+        if (t >= NEDGE) return;
+        const int slot = (p - z0 + 2) & 3;
+        if (t < NPX) {
+            const int c4 = t / RH, ryi = t % RH;
+            const int rx = c4 == 0 ? -1 : (c4 == 1 ? 0 : (c4 == 2 ? TX - 1 : TX));
+            const int pos = ryi * RW + rx + 1;
+            const bool hasy = ryi < 2 || ryi >= TY;
+            const int r4 = ryi < 2 ? ryi : ryi - (TY - 2);
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                T v = ring[(slot * 2 + k) * RS + pos] + stage[k * NPIECE + t];
+                if (hasy) { v += stage[k * NPIECE + NPX + r4 * RW + rx + 1]; v += stage[k * NPIECE + NPX + NPY + r4 * 4 + c4]; }
+                ring[(slot * 2 + k) * RS + pos] = v;
+            }
+        } else {
+            const int q = t - NPX, r4 = q / (RW - 4), rx = q % (RW - 4) + 1;
+            const int ry = r4 == 0 ? -1 : (r4 == 1 ? 0 : (r4 == 2 ? TY - 1 : TY));
+            const int pos = (ry + 1) * RW + rx + 1;
+#pragma unroll
+            for (int k = 0; k < 2; ++k) ring[(slot * 2 + k) * RS + pos] += stage[k * NPIECE + NPX + r4 * RW + rx + 1];
         }
     };
 
-    {
-        T v[4];
-#pragma unroll 1
-        for (int p = z0 - 2; p <= z0; ++p) { ring_load(p, v); ring_store(p, v); }
-    }
-    __syncthreads();
+    // ---- pulls ------------------------------------------------------------------------------------
+    // f_i(x) = h_i(x - c_i), or h_opp(i)(x) across a solid link
+    auto src_of = [&](int k, int i, const long long (&zoff)[3], long long n, unsigned lk) -> const T* {
+        const T* base = h + (long long)(k * Q) * NP;
+        if (HAS_SOLID && i > 0 && (lk >> dir_opp(i) & 1u)) return base + (long long)dir_opp(i) * NP + n;
+        return base + (long long)i * NP + zoff[1 - dir_cz(i)] + ys[1 - dir_cy(i)] + xs[1 - dir_cx(i)];
+    };
+    auto plane_of = [&](int p, long long (&zoff)[3], long long& n, unsigned& lk) {
+        zoff[0] = wrapz(p - 1) * pl; zoff[1] = wrapz(p) * pl; zoff[2] = wrapz(p + 1) * pl;
+        n = zoff[1] + own_xy;
+        lk = HAS_SOLID ? __ldg(links + n) : 0u;
+    };
+    auto prefetch_blue = [&](int p) {                          // -> stash, asynchronously
+        long long zoff[3], n; unsigned lk;
+        plane_of(p, zoff, n, lk);
+        if (!HAS_SOLID || !(lk & OP_SOLID_BIT)) {
+#pragma unroll
+            for (int i = 0; i < Q; ++i) cp_async<sizeof(T)>(stash + i * NT + t, src_of(1, i, zoff, n, lk));
+        }
+        cp_async_commit();
+    };
+    auto prefetch_red = [&](int p, T (&fr)[Q]) {               // -> registers
+        long long zoff[3], n; unsigned lk;
+        plane_of(p, zoff, n, lk);
+        if (!HAS_SOLID || !(lk & OP_SOLID_BIT)) {
+#pragma unroll
+            for (int i = 0; i < Q; ++i) fr[i] = __ldg(src_of(0, i, zoff, n, lk));
+        }
+    };
 
-    // z pipelines of the density partial sums: [k][0] = A_+1(z-1) + A_0(z) so far, [k][1] = A_+1(z)
+    // ---- prologue -----------------------------------------------------------------------------
+    T fr[Q];
+#pragma unroll
+    for (int i = 0; i < Q; ++i) fr[i] = T(0);
+    prefetch_red(z0 - 1, fr);
+    __syncthreads();                                           // zero fill done before anything lands in `stage`
+#pragma unroll 1
+    for (int p = z0 - 2; p <= z0; ++p) {
+        ring_issue(p);
+        cp_async_wait<0>();
+        __syncthreads();
+        ring_assemble(p);
+        __syncthreads();
+    }
+    prefetch_blue(z0 - 1);
+
+    // z pipelines of this node's density partial sums: [k][0] = A_+1(z-1) + A_0(z) so far, [k][1] = A_+1(z)
     T own_acc[2][2] = {{T(0), T(0)}, {T(0), T(0)}};
-    T halo_acc[2][2] = {{T(0), T(0)}, {T(0), T(0)}};
+
+    const T zero = T(0);
+    auto from_left = [&](T v) { const T r = __shfl_up_sync(0xffffffffu, v, 1); return tx == 0 ? zero : r; };
+    auto from_right = [&](T v) { const T r = __shfl_down_sync(0xffffffffu, v, 1); return tx == TX - 1 ? zero : r; };
 
 #pragma unroll 1
     for (int z = z0 - 1; z <= z1; ++z) {
-        const int zt = wrapz(z - 1);                             // plane index of the density target
-        const long long zoff[3] = {zt * pl, wrapz(z) * pl, wrapz(z + 1) * pl};
-        const long long n = zoff[1] + own_xy;
+        const int zt = wrapz(z - 1), zl = wrapz(z);              // plane of the density target / of this plane
+        const long long n = zl * pl + own_xy;
         const bool store_h = z >= z0 && z < z1;                 // planes z0-1 and z1 are re-collided only
         const bool store_rho = z - 1 >= z0;                     // target plane z-1 (always < z1 here)
+        const bool more = z < z1;                               // iteration z+1 exists
         const int s0 = (z - z0 + 2) & 3;                        // ring slot of plane z
         unsigned lk = 0;
         if (HAS_SOLID) lk = __ldg(links + n);
         const bool fluid = !HAS_SOLID || !(lk & OP_SOLID_BIT);  // nothing happens inside a particle
 
-        // pull the 19 populations of component k arriving at this node (Eq. 5 / Eq. 23-24)
-        auto pull = [&](int k, T (&fk)[Q]) {
-            const T* base = h + (long long)(k * Q) * NP;
-#pragma unroll
-            for (int i = 0; i < Q; ++i) {
-                const T* src = base + (long long)i * NP + zoff[1 - dir_cz(i)] + ys[1 - dir_cy(i)] + xs[1 - dir_cx(i)];
-                if (HAS_SOLID && i > 0 && (lk >> dir_opp(i) & 1u)) src = base + (long long)dir_opp(i) * NP + n;
-                fk[i] = __ldg(src);
+        // x stage of the density gather for one opposite pair (h1 = direction 2p+1, h2 = 2p+2) of component k:
+        // row sums into u0/up/um[cz+1], the tile's virtual columns -1 / TX into shared memory.
+        auto xpair = [&](int k, int p, T h1, T h2, T (&u0)[3], T (&up)[3], T (&um)[3]) {
+            T* sup0 = SU + (k * 6 + 1) * RS;                    // Up[dz = 0] plane
+            T* sum0 = SU + (k * 6 + 4) * RS;                    // Um[dz = 0] plane
+            T* e0k = e0a + k * 6 * TY;                          // [dz+1][side][TY]
+            T l = zero, r = zero;
+            if (p == 0 || (p >= 3 && p <= 6)) { l = from_left(h1); r = from_right(h2); }   // p is uniform: every lane shuffles
+            if (p == 0) {                                       // +x / -x
+                u0[1] += l; u0[1] += r;
+                if (tx == TX - 1) e0k[(1 * 2 + 1) * TY + ty] = h1;
+                if (tx == 0) e0k[(1 * 2 + 0) * TY + ty] = h2;
+            } else if (p == 1) { up[1] = h1; um[1] = h2; }       // +y / -y
+            else if (p == 2) { u0[2] = h1; u0[0] = h2; }         // +z / -z
+            else if (p == 3) {                                  // +x+y / -x-y
+                up[1] += l; um[1] += r;
+                if (tx == TX - 1) sup0[own_r + 1] = h1;
+                if (tx == 0) sum0[own_r - 1] = h2;
+            } else if (p == 4) {                                // +x-y / -x+y
+                um[1] += l; up[1] += r;
+                if (tx == TX - 1) sum0[own_r + 1] = h1;
+                if (tx == 0) sup0[own_r - 1] = h2;
+            } else if (p == 5) {                                // +x+z / -x-z
+                u0[2] += l; u0[0] += r;
+                if (tx == TX - 1) e0k[(2 * 2 + 1) * TY + ty] = h1;
+                if (tx == 0) e0k[(0 * 2 + 0) * TY + ty] = h2;
+            } else if (p == 6) {                                // +x-z / -x+z
+                u0[0] += l; u0[2] += r;
+                if (tx == TX - 1) e0k[(0 * 2 + 1) * TY + ty] = h1;
+                if (tx == 0) e0k[(2 * 2 + 0) * TY + ty] = h2;
+            } else if (p == 7) { up[2] = h1; um[0] = h2; }       // +y+z / -y-z
+            else { up[0] = h1; um[2] = h2; }                     // +y-z / -y+z
+            // corner exports: only cz = 0 directions reach a diagonal tile, so target plane = this plane
+            if (store_h && (p == 3 || p == 4)) {
+                if (p == 3 && tx == TX - 1 && ty == TY - 1) ro.xy[k * ro.s_xy + zl * psxy + (btyp * ntx + btxp) * 4 + 0] = h1;
+                if (p == 3 && tx == 0 && ty == 0) ro.xy[k * ro.s_xy + zl * psxy + (btym * ntx + btxm) * 4 + 3] = h2;
+                if (p == 4 && tx == TX - 1 && ty == 0) ro.xy[k * ro.s_xy + zl * psxy + (btym * ntx + btxp) * 4 + 2] = h1;
+                if (p == 4 && tx == 0 && ty == TY - 1) ro.xy[k * ro.s_xy + zl * psxy + (btyp * ntx + btxm) * 4 + 1] = h2;
             }
         };
-        // exchange the post-collision values and gather this step's contribution to rho(t+1)
-        auto publish = [&](const T (&fk)[Q]) {
+        // publish the y-stage inputs of component k and export across the tile's y edges
+        auto publish = [&](int k, const T (&up)[3], const T (&um)[3]) {
 #pragma unroll
-            for (int i = 1; i < Q; ++i)
-                if (!dir_local(i)) S[sidx(i) * PS + own_p] = fk[i];
-        };
-        auto gather = [&](int k, const T (&fk)[Q]) {
-            T a[3] = {T(0), T(0), T(0)};                         // index cz + 1
-#pragma unroll
-            for (int i = 0; i < Q; ++i)
-                a[dir_cz(i) + 1] += dir_local(i) ? fk[i] : S[sidx(i) * PS + own_p - dir_cy(i) * PW - dir_cx(i)];
-            if (HAS_SOLID) {                                     // bounced-back arrivals come from this node itself
-#pragma unroll
-                for (int i = 1; i < Q; ++i)
-                    if (lk >> dir_opp(i) & 1u) a[1] += fk[dir_opp(i)];
+            for (int d = 0; d < 3; ++d) {
+                SU[(k * 6 + d) * RS + own_r] = up[d];
+                SU[(k * 6 + 3 + d) * RS + own_r] = um[d];
             }
-            const T out = own_acc[k][0] + a[0];
-            own_acc[k][0] = own_acc[k][1] + a[1];
-            own_acc[k][1] = a[2];
-            if (store_rho) ro.in[k * ro.s_in + zoff[0] + own_xy] = out;
-            if (has_halo) {
-                T b[3] = {T(0), T(0), T(0)};
-#pragma unroll
-                for (int i = 1; i < Q; ++i)
-                    if (!dir_local(i)) b[dir_cz(i) + 1] += S[sidx(i) * PS + halo_p - dir_cy(i) * PW - dir_cx(i)];
-                const T hout = halo_acc[k][0] + b[0];
-                halo_acc[k][0] = halo_acc[k][1] + b[1];
-                halo_acc[k][1] = b[2];
-                if (store_rho) {
-                    if (halo_corner) ro.xy[k * ro.s_xy + zt * psxy + halo_oxy] = hout;
-                    else if (halo_col) ro.x[k * ro.s_x + zt * psx + halo_ox] = hout;
-                    else ro.y[k * ro.s_y + zt * psy + halo_oy] = hout;
-                }
+            if (ty == 0 || ty == TY - 1) {                      // the row beyond the edge receives exactly Um (Up)
+                const int which = ty == 0 ? 0 : 1;
+                T* acc = accr + ((k * 2 + which) * TX + tx) * 2;
+                const T a_m = which == 0 ? um[0] : up[0], a_0 = which == 0 ? um[1] : up[1], a_p = which == 0 ? um[2] : up[2];
+                const T out = acc[0] + a_m;
+                acc[0] = acc[1] + a_0;
+                acc[1] = a_p;
+                if (store_rho) ro.y[k * ro.s_y + zt * psy + ((which == 0 ? btym : btyp) * 2 + (which == 0 ? 1 : 0)) * nx + x] = out;
             }
         };
 
-        T fk[Q];
-        T rb = T(0), ux = T(0), uy = T(0), uz = T(0);
-        T eb[3] = {T(0), T(0), T(0)};
+        // ---- moments of both components, common velocity, force --------------------------------
+        cp_async_wait<0>();                                      // this thread's stash slots have landed
+        T rr = T(0), rb = T(0), ux = T(0), uy = T(0), uz = T(0);
+        T er[3] = {T(0), T(0), T(0)}, eb[3] = {T(0), T(0), T(0)};
         if (fluid) {
-            T jb[3], jr[3], rr;
-            pull(1, fk);
-            moments19<T>(fk, rb, jb[0], jb[1], jb[2]);
-            pull(0, fk);
-            moments19<T>(fk, rr, jr[0], jr[1], jr[2]);
-            const T den = om_r * rr + om_b * rb;                 // S4
-            const T inv = den != T(0) ? T(1) / den : T(0);
-            ux = (om_r * jr[0] + om_b * jb[0]) * inv;
-            uy = (om_r * jr[1] + om_b * jb[1]) * inv;
-            uz = (om_r * jr[2] + om_b * jb[2]) * inv;
+            T jb[3] = {T(0), T(0), T(0)}, jr[3];
+            rb = stash[t];
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                const T a = stash[(2 * p + 1) * NT + t], b = stash[(2 * p + 2) * NT + t];
+                rb += a + b;
+                const T d = a - b;
+                if (pair_cx(p)) jb[0] += T(pair_cx(p)) * d;
+                if (pair_cy(p)) jb[1] += T(pair_cy(p)) * d;
+                if (pair_cz(p)) jb[2] += T(pair_cz(p)) * d;
+            }
             // du^k = -G sum_i w_i rho^kbar(x+c_i) c_i (S2, S3, S6); a solid neighbour counts 0 (S7)
             T gr[3] = {T(0), T(0), T(0)}, gb[3] = {T(0), T(0), T(0)};
 #pragma unroll
             for (int p = 0; p < 9; ++p) {
-                const int sp = (s0 + pair_cz(p)) & 3, sm = (s0 - pair_cz(p)) & 3;
+                const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
                 const int op = own_r + pair_cy(p) * RW + pair_cx(p), om = own_r - pair_cy(p) * RW - pair_cx(p);
-                T bp = ring[(sp * 2 + 1) * RS + op], bm = ring[(sm * 2 + 1) * RS + om];
-                T rp = ring[(sp * 2 + 0) * RS + op], rm = ring[(sm * 2 + 0) * RS + om];
+                T bp = ring[(sp * 2 + 1) * RS + op], bm = ring[(sm_ * 2 + 1) * RS + om];
+                T rp = ring[(sp * 2 + 0) * RS + op], rm = ring[(sm_ * 2 + 0) * RS + om];
                 if (HAS_SOLID) {
                     if (lk >> (2 * p + 1) & 1u) { bp = T(0); rp = T(0); }
                     if (lk >> (2 * p + 2) & 1u) { bm = T(0); rm = T(0); }
@@ -253,36 +357,113 @@ k_step_pull(const T* __restrict__ h, T* __restrict__ g, const unsigned* __restri
                 if (pair_cy(p)) { gr[1] += T(pair_cy(p)) * db; gb[1] += T(pair_cy(p)) * dr; }
                 if (pair_cz(p)) { gr[2] += T(pair_cz(p)) * db; gb[2] += T(pair_cz(p)) * dr; }
             }
+            moments19<T>(fr, rr, jr[0], jr[1], jr[2]);
+            const T den = om_r * rr + om_b * rb;                 // S4
+            const T inv = den != T(0) ? T(1) / den : T(0);
+            ux = (om_r * jr[0] + om_b * jb[0]) * inv;
+            uy = (om_r * jr[1] + om_b * jb[1]) * inv;
+            uz = (om_r * jr[2] + om_b * jb[2]) * inv;
+            er[0] = ux - G * gr[0]; er[1] = uy - G * gr[1]; er[2] = uz - G * gr[2];
             eb[0] = ux - G * gb[0]; eb[1] = uy - G * gb[1]; eb[2] = uz - G * gb[2];
-            collide19<T>(fk, rr, T(1) - om_r, ux, uy, uz, ux - G * gr[0], uy - G * gr[1], uz - G * gr[2]);
-            if (store_h) {
-#pragma unroll
-                for (int i = 0; i < Q; ++i) g[(long long)i * NP + n] = fk[i];
-            }
-        } else {
-#pragma unroll
-            for (int i = 0; i < Q; ++i) fk[i] = T(0);
         }
-        publish(fk);
-        __syncthreads();
-        gather(0, fk);
+        if (more) ring_issue(z + 2);                             // slot of plane z-2: last read one iteration ago
+
+        // ---- blue: collide pair by pair out of the stash, store, x stage, publish -----------------
+        T u0b[3] = {T(0), T(0), T(0)};
+        {
+            T up[3] = {T(0), T(0), T(0)}, um[3] = {T(0), T(0), T(0)};
+            const T omc = T(1) - om_b;
+            const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+            const T ae = T(1) - T(1.5) * (eb[0] * eb[0] + eb[1] * eb[1] + eb[2] * eb[2]);
+            T* o = g + (long long)Q * NP + n;
+            T bs = T(0);
+            {
+                const T h0 = fluid ? omc * stash[t] + w_rest<T>() * rb * (ae - omc * a0) : zero;
+                if (fluid && store_h) o[0] = h0;
+                u0b[1] = h0;
+            }
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                T h1 = zero, h2 = zero;
+                if (fluid) {
+                    const T cu = T(pair_cx(p)) * ux + T(pair_cy(p)) * uy + T(pair_cz(p)) * uz;
+                    const T ce = T(pair_cx(p)) * eb[0] + T(pair_cy(p)) * eb[1] + T(pair_cz(p)) * eb[2];
+                    const T wr = w_pair<T>(p) * rb;
+                    const T sym = wr * ((ae + T(4.5) * ce * ce) - omc * (a0 + T(4.5) * cu * cu));
+                    const T asym = (T(3) * wr) * (ce - omc * cu);
+                    h1 = omc * stash[(2 * p + 1) * NT + t] + (sym + asym);
+                    h2 = omc * stash[(2 * p + 2) * NT + t] + (sym - asym);
+                    if (store_h) { o[(long long)(2 * p + 1) * NP] = h1; o[(long long)(2 * p + 2) * NP] = h2; }
+                    if (HAS_SOLID) {                             // bounced-back arrivals of the next step come from this node
+                        if (lk >> (2 * p + 1) & 1u) bs += h1;
+                        if (lk >> (2 * p + 2) & 1u) bs += h2;
+                    }
+                }
+                xpair(1, p, h1, h2, u0b, up, um);
+            }
+            if (HAS_SOLID) u0b[1] += bs;
+            publish(1, up, um);
+        }
+        if (more) prefetch_blue(z + 1);
+
+        // ---- red: collide out of the registers, store, x stage, publish ---------------------------
+        T u0r[3] = {T(0), T(0), T(0)};
+        {
+            T up[3] = {T(0), T(0), T(0)}, um[3] = {T(0), T(0), T(0)};
+            T bs = T(0);
+            if (fluid) {
+                collide19<T>(fr, rr, T(1) - om_r, ux, uy, uz, er[0], er[1], er[2]);
+                if (store_h) {
+#pragma unroll
+                    for (int i = 0; i < Q; ++i) g[(long long)i * NP + n] = fr[i];
+                }
+                if (HAS_SOLID) {
+#pragma unroll
+                    for (int i = 1; i < Q; ++i)
+                        if (lk >> i & 1u) bs += fr[i];
+                }
+            }
+            u0r[1] = fluid ? fr[0] : zero;
+#pragma unroll
+            for (int p = 0; p < 9; ++p) xpair(0, p, fluid ? fr[2 * p + 1] : zero, fluid ? fr[2 * p + 2] : zero, u0r, up, um);
+            if (HAS_SOLID) u0r[1] += bs;
+            publish(0, up, um);
+        }
+        if (more) {
+            prefetch_red(z + 1, fr);
+            cp_async_wait<1>();                                  // the ring pieces of plane z+2 (the stash may still fly)
+        }
         __syncthreads();
 
-        T rv[4];
-        const bool fill = z < z1;                                // plane z+2 is needed by iteration z+1
-        if (fill) ring_load(z + 2, rv);
-        if (fluid) {
-            pull(1, fk);
-            collide19<T>(fk, rb, T(1) - om_b, ux, uy, uz, eb[0], eb[1], eb[2]);
-            if (store_h) {
+        // ---- y stage and z pipeline of the gather; exports across the tile's x edges ---------------
 #pragma unroll
-                for (int i = 0; i < Q; ++i) g[(long long)(Q + i) * NP + n] = fk[i];
+        for (int k = 0; k < 2; ++k) {
+            const T* u0 = k == 0 ? u0r : u0b;
+            T a[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                a[d] = u0[d] + SU[(k * 6 + d) * RS + own_r - RW];          // Up[dz](y-1)
+                a[d] += SU[(k * 6 + 3 + d) * RS + own_r + RW];             // Um[dz](y+1)
+            }
+            const T out = own_acc[k][0] + a[0];
+            own_acc[k][0] = own_acc[k][1] + a[1];
+            own_acc[k][1] = a[2];
+            if (store_rho) ro.in[k * ro.s_in + (long long)zt * pl + own_xy] = out;
+            if (tx == 0 || tx == TX - 1) {
+                const int side = tx == 0 ? 0 : 1;
+                const int vc = tx == 0 ? own_r - 1 : own_r + 1;            // the virtual column next to this lane
+                const T* e0k = e0a + k * 6 * TY;
+                T a_0 = e0k[(1 * 2 + side) * TY + ty] + SU[(k * 6 + 1) * RS + vc - RW];
+                a_0 += SU[(k * 6 + 4) * RS + vc + RW];
+                const T a_m = e0k[(0 * 2 + side) * TY + ty], a_p = e0k[(2 * 2 + side) * TY + ty];
+                T* acc = accc + ((k * 2 + side) * TY + ty) * 2;
+                const T hout = acc[0] + a_m;
+                acc[0] = acc[1] + a_0;
+                acc[1] = a_p;
+                if (store_rho) ro.x[k * ro.s_x + zt * psx + ((bty * ntx + (side == 0 ? btxm : btxp)) * 2 + (side == 0 ? 1 : 0)) * TY + ty] = hout;
             }
         }
-        publish(fk);
-        if (fill) ring_store(z + 2, rv);
-        __syncthreads();
-        gather(1, fk);
+        if (more) ring_assemble(z + 2);
         __syncthreads();
     }
 }
