@@ -217,12 +217,12 @@ def run_ours(args):
 
     stream = torch.cuda.Stream(device=dev)
     box = B.Box(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype, cuda_stream=stream.cuda_stream)
-    kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS}[args.kernel]
+    kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA}[args.kernel]
     box.set_kernel(kernel)
     if mask is not None:
         box.set_solid_mask(mask)
     box.set_fields(rr, rb)
-    kname = B.lb_kernel_name(box.h) if hasattr(B, "lb_kernel_name") else args.kernel
+    kname = B.lb_kernel_name(box.h)
 
     # ---- device-resident timing: K steps between two events on the launching stream ----
     box.step(warmup)
@@ -303,7 +303,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS))
-    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     return run_reference(args) if args.impl == "reference" else run_ours(args)

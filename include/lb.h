@@ -42,7 +42,7 @@ typedef struct lb_ctx lb_ctx;          /* opaque; owned by the library */
 
 enum { LB_OK = 0, LB_EINVAL = -1, LB_ENOMEM = -2, LB_ECUDA = -3, LB_ESTATE = -4 };
 enum { LB_F64 = 0, LB_F32 = 1 };
-enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2 };
+enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2, LB_KERNEL_TMA = 3 };
 
 /* Create a context for an nx*ny*nz periodic box holding two fluids with BGK
  * relaxation times tau_r, tau_b (Eq. 1; omega_k = 1/tau_k) coupled by the
@@ -112,9 +112,14 @@ int lb_get_diagnostics(lb_ctx* ctx, double mass[2], double momentum[3]);
 
 /* Choose the time-step kernel: LB_KERNEL_TWOPASS = density pass + fused collide/stream pass
  * (reads the populations twice per step); LB_KERNEL_ONEPASS = single fused pass that
- * reads and writes every population once per step; LB_KERNEL_AUTO (default) = ONEPASS when
- * the box shape allows it, else TWOPASS.  LB_EINVAL if the box shape does not allow `kind`. */
+ * reads and writes every population once per step, populations pulled with per-thread loads;
+ * LB_KERNEL_TMA = the same single pass with the populations staged in shared memory by the TMA
+ * unit (the fastest; needs nx % 32 == 0 and ny % 8 == 0 like ONEPASS); LB_KERNEL_AUTO (default) =
+ * TMA when the box shape allows it, else TWOPASS.  LB_EINVAL if the box shape does not allow `kind`. */
 int lb_set_kernel(lb_ctx* ctx, int kind);
+
+/* The kernel lb_step will use (LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS or LB_KERNEL_TMA; never AUTO); -1 for a NULL context. */
+int lb_get_kernel(const lb_ctx* ctx);
 
 /* Number of kernel launches this context has enqueued so far (for bench.py's gpu_launches). */
 long long lb_launch_count(const lb_ctx* ctx);

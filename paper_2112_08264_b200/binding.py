@@ -16,7 +16,7 @@ import numpy as np
 
 LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 LB_F64, LB_F32 = 0, 1
-LB_KERNEL_AUTO, LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS = 0, 1, 2
+LB_KERNEL_AUTO, LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA = 0, 1, 2, 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "_lib", "liblb_b200.so")
@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_HERE, "_lib", "liblb_b200.so")
 SYMBOLS = (
     "lb_create", "lb_create_ex", "lb_destroy", "lb_set_fields", "lb_set_solid_mask",
     "lb_set_populations", "lb_step", "lb_get_populations", "lb_get_moments",
-    "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_launch_count",
+    "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
     "lb_sync", "lb_last_error", "lb_version",
 )
 
@@ -66,6 +66,7 @@ def lib() -> C.CDLL:
     L.lb_set_kernel.argtypes = [C.c_void_p, C.c_int]
     L.lb_launch_count.restype = C.c_longlong
     L.lb_launch_count.argtypes = [C.c_void_p]
+    L.lb_get_kernel.argtypes = [C.c_void_p]
     L.lb_sync.argtypes = [C.c_void_p]
     L.lb_last_error.restype = C.c_char_p
     L.lb_version.restype = C.c_char_p
@@ -164,6 +165,13 @@ def lb_get_diagnostics(h):
 
 def lb_set_kernel(h, kind):
     _chk(lib().lb_set_kernel(h, kind))
+
+
+KERNEL_NAMES = {LB_KERNEL_TWOPASS: "twopass", LB_KERNEL_ONEPASS: "onepass", LB_KERNEL_TMA: "tma"}
+
+
+def lb_kernel_name(h) -> str:
+    return KERNEL_NAMES.get(int(lib().lb_get_kernel(h)), "?")
 
 
 def lb_launch_count(h) -> int:

@@ -20,6 +20,7 @@
 #include "../../include/lb.h"
 #include "lb_lattice.cuh"
 #include "lb_onepass.cuh"
+#include "lb_tma.cuh"
 
 using namespace lb;
 
@@ -48,6 +49,8 @@ struct lb_ctx {
     int kernel;        // resolved LB_KERNEL_*
     int kernel_req;
     int zc;            // planes per CTA of the one-pass kernel
+    CUtensorMap tmap[2][2];   // [buffer][narrow box 32 x TY, wide box (32 + 16 B) x TY] over [k*19+i][z][y][x]
+    bool have_tmap;
     double* stage;     // device staging, STAGE_NODES * 5 doubles
     double* diag_part; // [DIAG_BLOCKS][5]
     double* diag_out;  // [5]
@@ -509,9 +512,72 @@ int step_onepass(lb_ctx* c) {
     return LB_OK;
 }
 
+// ----------------------------------------------------------------------------------------
+// TMA-staged one-pass time step (lb_tma.cuh): same boxes, same density arrays as the one-pass kernel
+// ----------------------------------------------------------------------------------------
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+// tensor maps over the population buffers: dims (x, y, z, plane), one box = one tile row block of one plane
+bool make_tmaps(lb_ctx* c) {
+    EncodeTiledFn enc = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", reinterpret_cast<void**>(&enc), cudaEnableDefault, &qr) != cudaSuccess || !enc) {
+        cudaGetLastError();
+        return false;
+    }
+    const cuuint64_t es = esize(c);
+    const cuuint64_t gdim[4] = {cuuint64_t(c->nx), cuuint64_t(c->ny), cuuint64_t(c->nz), cuuint64_t(NPOP)};
+    const cuuint64_t gstr[3] = {cuuint64_t(c->nx) * es, cuuint64_t(c->nx) * c->ny * es, cuuint64_t(c->NP) * es};
+    const cuuint32_t estr[4] = {1, 1, 1, 1};
+    const CUtensorMapDataType dt = c->dtype == LB_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    for (int b = 0; b < 2; ++b)
+        for (int w = 0; w < 2; ++w) {
+            const cuuint32_t box[4] = {cuuint32_t(OP_TX + (w ? 16 / int(es) : 0)), cuuint32_t(OP_TY), 1, 1};
+            if (enc(&c->tmap[b][w], dt, 4, c->f[b], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+                return false;
+        }
+    return true;
+}
+
+template <typename T, bool HAS_SOLID>
+int launch_tma(lb_ctx* c) {
+    auto kern = k_step_tma<T, HAS_SOLID, OP_TY>;
+    constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
+    static bool configured = false;                         // per instantiation
+    if (!configured) {
+        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
+        configured = true;
+    }
+    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc - 1) / c->zc);
+    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
+    kern<<<grid, OP_TX * OP_TY + 32, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], static_cast<const T*>(c->f[c->cur]),
+                                                        static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
+                                                        rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
+                                                        c->zc, om_r, om_b, G);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return LB_OK;
+}
+
+template <typename T>
+int step_tma(lb_ctx* c) {
+    int rc = ensure_rho<T>(c);
+    if (rc != LB_OK) return rc;
+    rc = c->has_solid ? launch_tma<T, true>(c) : launch_tma<T, false>(c);
+    if (rc != LB_OK) return rc;
+    c->cur ^= 1;
+    c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
+    return LB_OK;
+}
+
 int resolve_kernel(lb_ctx* c, int kind) {
-    if (kind == LB_KERNEL_AUTO) return onepass_ok(c) ? LB_KERNEL_ONEPASS : LB_KERNEL_TWOPASS;
+    const bool tma_ok = onepass_ok(c) && c->have_tmap;
+    if (kind == LB_KERNEL_AUTO) return tma_ok ? LB_KERNEL_TMA : (onepass_ok(c) ? LB_KERNEL_ONEPASS : LB_KERNEL_TWOPASS);
     if (kind == LB_KERNEL_ONEPASS && !onepass_ok(c)) return -1;
+    if (kind == LB_KERNEL_TMA && !tma_ok) return -1;
     return kind;
 }
 
@@ -588,6 +654,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
         lb_destroy(c);
         return nullptr;                                  // LB_ENOMEM
     }
+    c->have_tmap = onepass_ok(c) && make_tmaps(c);
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
     c->zc = onepass_zc(c);
@@ -616,11 +683,13 @@ int lb_sync(lb_ctx* c) {
 
 long long lb_launch_count(const lb_ctx* c) { return c ? c->launches : 0; }
 
+int lb_get_kernel(const lb_ctx* c) { return c ? c->kernel : -1; }
+
 int lb_set_kernel(lb_ctx* c, int kind) {
     if (!c) return fail(LB_EINVAL, "NULL context");
-    if (kind != LB_KERNEL_AUTO && kind != LB_KERNEL_TWOPASS && kind != LB_KERNEL_ONEPASS) return fail(LB_EINVAL, "unknown kernel kind");
+    if (kind != LB_KERNEL_AUTO && kind != LB_KERNEL_TWOPASS && kind != LB_KERNEL_ONEPASS && kind != LB_KERNEL_TMA) return fail(LB_EINVAL, "unknown kernel kind");
     const int r = resolve_kernel(c, kind);
-    if (r < 0) return fail(LB_EINVAL, "box shape does not allow the one-pass kernel");
+    if (r < 0) return fail(LB_EINVAL, "box shape does not allow this kernel");
     c->kernel_req = kind;
     c->kernel = r;
     return LB_OK;
@@ -719,7 +788,8 @@ int lb_step(lb_ctx* c, int nsteps) {
     if (!c->have_fields) return fail(LB_ESTATE, "lb_step before lb_set_fields / lb_set_populations");
     for (int s = 0; s < nsteps; ++s) {
         int rc;
-        if (c->kernel == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);
+        if (c->kernel == LB_KERNEL_TMA) rc = c->dtype == LB_F64 ? step_tma<double>(c) : step_tma<float>(c);
+        else if (c->kernel == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);
         else rc = c->dtype == LB_F64 ? step_twopass<double>(c) : step_twopass<float>(c);
         if (rc != LB_OK) return rc;
     }

@@ -1,0 +1,444 @@
+// lb_tma.cuh -- the fused one-pass time step with TMA-staged populations (the hot kernel on B200).
+//
+// Same algorithm and same state convention as lb_onepass.cuh (h-state, pull streaming, density carried
+// from step to step through the four single-writer arrays rho_in / rho_x / rho_y / rho_xy), but the
+// 38 population planes of a tile are brought into shared memory by the TMA unit instead of by 38
+// per-thread loads:
+//   * one producer warp per CTA issues, per z plane, 38 `cp.async.bulk.tensor.4d` box loads (one per
+//     population plane, box = tile shifted by -c_i in y and z) that complete on an mbarrier; the TX*TY
+//     consumer threads then read their 38 values with immediate-offset LDS: no per-thread address
+//     arithmetic, no registers in flight, and the prefetch distance is a whole plane whatever the
+//     occupancy is;
+//   * measured on B200: a TMA box whose innermost start is not 16-byte aligned
+//     raises an illegal-instruction fault, so the x shift cannot be given to the TMA.  Directions with
+//     c_x != 0 are loaded as an ALIGNED box that is PADX = 16/sizeof(T) elements wider, and the consumer
+//     applies the shift in its LDS address (free);
+//   * the TMA zero-fills out-of-range box parts and does not wrap: in tiles that touch the
+//     box boundary in x or y the producer warp patches the wrapped column / row from global memory after
+//     the box has landed and releases the consumers through a second mbarrier.  z wraps in the
+//     coordinate;
+//   * consumers copy the stage into registers and release it at once, so one stage buffers a whole
+//     plane of prefetch; post-collision values are stored straight from registers (aligned, coalesced);
+//   * one named barrier per plane (the y stage of the density gather, double-buffered), none for the
+//     stage hand-off (mbarriers).
+//
+// One CTA = TX*TY consumer threads (one node each, one warp per tile row) + 1 producer warp.
+#pragma once
+#include <cuda.h>
+
+#include "lb_lattice.cuh"
+#include "lb_onepass.cuh"
+
+namespace lb {
+
+// ---- PTX wrappers ----------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return static_cast<unsigned>(__cvta_generic_to_shared(p)); }
+__device__ __forceinline__ void mbar_init(void* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(void* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(void* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred P1;\n\tLAB_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, 0x989680;\n\t"
+        "@P1 bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// box load: coordinates (x, y, z, plane); x * sizeof(T) must be a multiple of 16 (see header)
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
+template <int ID, int COUNT>
+__device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(COUNT) : "memory"); }
+
+// ---- shared-memory layout -----------------------------------------------------------------------------
+template <typename T, int TY>
+struct TmaLayout {
+    static constexpr int TX = 32, NT = TX * TY;
+    static constexpr int PADX = 16 / int(sizeof(T));                   // elements per 16 bytes
+    static constexpr int W = TX + PADX;                                // row length of a wide (c_x != 0) slot
+    static constexpr int RW = TX + 2, RH = TY + 2, RS = RW * RH;       // density ring plane: tile + one-node frame
+    static constexpr int SUP = TY * RW;                                // one y-stage plane: tile rows with an x frame
+    __host__ __device__ static constexpr int align128(int elems) { return (elems * int(sizeof(T)) + 127) / 128 * 128 / int(sizeof(T)); }
+    static constexpr int NA = align128(NT), WA = align128(W * TY);     // slot sizes: narrow (c_x = 0) and wide boxes, 128-byte multiples
+    // number of wide slots before direction i (the directions with c_x != 0 are 1, 2, 7..14)
+    __host__ __device__ static constexpr int wide_before(int i) { return (i > 1) + (i > 2) + (i > 7 ? (i - 7 < 8 ? i - 7 : 8) : 0); }
+    __host__ __device__ static constexpr int slot_off(int q) {         // element offset of population plane q = k*19 + i
+        return (q / Q) * (9 * NA + 10 * WA) + (q % Q - wide_before(q % Q)) * NA + wide_before(q % Q) * WA;
+    }
+    static constexpr int STAGE = 0;
+    static constexpr int STAGE_ELEMS = slot_off(NPOP);
+    static constexpr unsigned STAGE_TX_BYTES = unsigned(2 * (9 * NT + 10 * W * TY) * sizeof(T));   // bytes the 38 boxes deliver
+    static constexpr int RING = STAGE + STAGE_ELEMS;                   // [4][2][RS]      rho(t), planes z-1..z+2
+    static constexpr int SU = RING + 8 * RS;                           // [2][2][6][SUP]  double-buffered Up[dz], Um[dz] per component
+    static constexpr int END = SU + 24 * SUP;
+    static constexpr size_t BAR_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
+    static constexpr size_t BYTES = BAR_BYTE_OFF + 4 * sizeof(unsigned long long);
+    // where consumer (tx, ty) finds f_i = h_i(x - c_i) inside slot i
+    __host__ __device__ static constexpr int read_off(int i, int tx, int ty) {
+        return dir_cx(i) == 0 ? ty * TX + tx : ty * W + tx + (dir_cx(i) > 0 ? PADX - 1 : 1);
+    }
+};
+
+
+// ---- the kernel ------------------------------------------------------------------------------------------
+template <typename T, bool HAS_SOLID, int TY>
+__global__ void __launch_bounds__(32 * TY + 32, 1)
+k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
+           const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
+           const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
+           T om_r, T om_b, T G) {
+    using L = TmaLayout<T, TY>;
+    constexpr int TX = L::TX, NT = L::NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
+    static_assert(RS <= 2 * NT, "ring fill: at most two positions per consumer thread");
+    extern __shared__ __align__(1024) unsigned char smem_tma[];
+    T* sm = reinterpret_cast<T*>(smem_tma);
+    T* stage = sm + L::STAGE;
+    T* ring = sm + L::RING;
+    T* SUb = sm + L::SU;
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma + L::BAR_BYTE_OFF);
+    unsigned long long* full = bars;          // the 38 boxes of the next plane have landed (tx bytes)
+    unsigned long long* patch = bars + 1;     // ... and the producer has patched the wrapped column / row (boundary tiles)
+    unsigned long long* done = bars + 2;      // every consumer warp has copied the stage into registers
+
+    const int t = threadIdx.x;
+    const int ntx = nx / TX, nty = ny / TY;
+    const int btx = blockIdx.x, bty = blockIdx.y;
+    const int x0 = btx * TX, y0 = bty * TY;
+    const int z0 = blockIdx.z * zc;
+    const int z1 = min(z0 + zc, nz);
+    const int niter = z1 - z0 + 2;            // planes z0-1 .. z1; the first and the last are re-collided only
+    const long long pl = (long long)nx * ny;
+    const bool wrap_tile = btx == 0 || btx == ntx - 1 || bty == 0 || bty == nty - 1;
+    auto wrapz = [&](int p) { p %= nz; return p < 0 ? p + nz : p; };
+
+    if (t == 0) {
+        mbar_init(full, 1);
+        mbar_init(patch, 1);
+        mbar_init(done, TY);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // =================================== producer warp ===================================
+    if (t >= NT) {
+        const int lane = t - NT;
+        for (int j = 0; j < niter; ++j) {
+            const int z = z0 - 1 + j;
+            const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
+            if (lane == 0) {
+                if (j > 0) mbar_wait(done, (j - 1) & 1);
+                mbar_expect_tx(full, L::STAGE_TX_BYTES);
+#pragma unroll
+                for (int q = 0; q < NPOP; ++q) {
+                    const int i = q % Q;
+                    const int zq = zw[1 - dir_cz(i)];                       // f_i(x) = h_i(x - c_i)
+                    if (dir_cx(i) == 0) tma_load_4d(stage + L::slot_off(q), &tm_n, full, x0, y0 - dir_cy(i), zq, q);
+                    else tma_load_4d(stage + L::slot_off(q), &tm_w, full, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zq, q);
+                }
+            }
+            __syncwarp();
+            if (wrap_tile) {                                                // the TMA zero-filled what lies outside the box
+                mbar_wait(full, j & 1);
+#pragma unroll
+                for (int q = 0; q < NPOP; ++q) {
+                    const int i = q % Q;
+                    const int cx = dir_cx(i), cy = dir_cy(i);
+                    if (cx == 0 && cy == 0) continue;
+                    const T* src = h + (long long)q * NP + (long long)zw[1 - dir_cz(i)] * pl;
+                    T* slot = stage + L::slot_off(q);
+                    const int rowlen = cx == 0 ? TX : W;
+                    const int ox = cx > 0 ? x0 - PADX : x0;                 // global x of slot column 0
+                    if (cx != 0 && ((cx > 0 && btx == 0) || (cx < 0 && btx == ntx - 1))) {
+                        const int col = cx > 0 ? PADX - 1 : TX;             // the one column a consumer reads outside [0, nx)
+                        const int gx = cx > 0 ? nx - 1 : 0;
+                        if (lane < TY) {
+                            int gy = y0 - cy + lane;
+                            gy = gy < 0 ? gy + ny : (gy >= ny ? gy - ny : gy);
+                            slot[lane * rowlen + col] = src[(long long)gy * nx + gx];
+                        }
+                    }
+                    if (cy != 0 && ((cy > 0 && bty == 0) || (cy < 0 && bty == nty - 1))) {
+                        const int row = cy > 0 ? 0 : TY - 1;
+                        const int gy = cy > 0 ? ny - 1 : 0;
+                        for (int c = lane; c < rowlen; c += 32) {
+                            int gx = ox + c;
+                            gx = gx < 0 ? gx + nx : (gx >= nx ? gx - nx : gx);
+                            slot[row * rowlen + c] = src[(long long)gy * nx + gx];
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(patch);
+            }
+        }
+        return;
+    }
+
+    // =================================== consumers ===================================
+    const int tx = t % TX, ty = t / TX;
+    const int x = x0 + tx, y = y0 + ty;
+    const int own_xy = y * nx + x;
+    const int own_r = (ty + 1) * RW + tx + 1;                              // ring position (tile + frame)
+    const int own_s = ty * RW + tx + 1;                                    // y-stage plane position (x frame only)
+    const long long psx = (long long)nty * ntx * 2 * TY, psy = (long long)nty * 2 * nx, psxy = (long long)nty * ntx * 4;
+    const int btxm = btx == 0 ? ntx - 1 : btx - 1, btxp = btx == ntx - 1 ? 0 : btx + 1;
+    const int btym = bty == 0 ? nty - 1 : bty - 1, btyp = bty == nty - 1 ? 0 : bty + 1;
+    const T zero = T(0);
+
+    // ---- density ring: every consumer owns ring positions t and t + NT and assembles them from the four
+    //      single-writer arrays in the fixed order ((in + x) + y) + xy ----
+    int o_in[2], o_x[2], o_y[2], o_xy[2];
+#pragma unroll
+    for (int a = 0; a < 2; ++a) {
+        const int pos = t + a * NT;
+        o_in[a] = o_x[a] = o_y[a] = o_xy[a] = -1;
+        if (pos < RS) {
+            const int rx = pos % RW - 1, ry = pos / RW - 1;
+            const int otx = rx < 0 ? btxm : (rx >= TX ? btxp : btx), oty = ry < 0 ? btym : (ry >= TY ? btyp : bty);
+            const int lx = rx < 0 ? TX - 1 : (rx >= TX ? 0 : rx), ly = ry < 0 ? TY - 1 : (ry >= TY ? 0 : ry);
+            const bool ex = lx == 0 || lx == TX - 1, ey = ly == 0 || ly == TY - 1;
+            o_in[a] = (oty * TY + ly) * nx + otx * TX + lx;
+            if (ex) o_x[a] = ((oty * ntx + otx) * 2 + (lx != 0)) * TY + ly;
+            if (ey) o_y[a] = (oty * 2 + (ly != 0)) * nx + otx * TX + lx;
+            if (ex && ey) o_xy[a] = (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
+        }
+    }
+    T raw[2][2][4];                                                        // [position][component][in, x, y, xy] of the plane in flight
+    auto ring_load = [&](int p) {
+        const long long zl = wrapz(p);
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                if (o_in[a] >= 0) raw[a][k][0] = __ldg(ri.in + k * ri.s_in + zl * pl + o_in[a]);
+                if (o_x[a] >= 0) raw[a][k][1] = __ldg(ri.x + k * ri.s_x + zl * psx + o_x[a]);
+                if (o_y[a] >= 0) raw[a][k][2] = __ldg(ri.y + k * ri.s_y + zl * psy + o_y[a]);
+                if (o_xy[a] >= 0) raw[a][k][3] = __ldg(ri.xy + k * ri.s_xy + zl * psxy + o_xy[a]);
+            }
+    };
+    auto ring_store = [&](int slot) {
+#pragma unroll
+        for (int a = 0; a < 2; ++a)
+#pragma unroll
+            for (int k = 0; k < 2; ++k) {
+                if (o_in[a] < 0) continue;
+                T v = raw[a][k][0];
+                if (o_x[a] >= 0) v += raw[a][k][1];
+                if (o_y[a] >= 0) v += raw[a][k][2];
+                if (o_xy[a] >= 0) v += raw[a][k][3];
+                ring[(slot * 2 + k) * RS + t + a * NT] = v;
+            }
+    };
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) raw[a][k][c] = zero;
+#pragma unroll 1
+    for (int p = 0; p < 3; ++p) {                                          // planes z0-2, z0-1, z0 -> slots 0, 1, 2
+        ring_load(z0 - 2 + p);
+        ring_store(p);
+    }
+    ring_load(z0 + 1);                                                     // stored in iteration 0
+    named_barrier<1, NT>();
+
+    // ---- per-thread state carried along z ----
+    T own_acc[2][2] = {{zero, zero}, {zero, zero}};     // z pipeline of this node's gathered density: [k][0] = A_+1(z-2) + A_0(z-1), [k][1] = A_+1(z-1)
+    T row_acc[2][2] = {{zero, zero}, {zero, zero}};     // the same for the export across the tile's y edge (warps ty = 0 and TY-1)
+    T col_acc[2][2] = {{zero, zero}, {zero, zero}};     // ... across the tile's x edge (lanes tx = 0 and TX-1)
+    auto from_left = [&](T v) { const T r = __shfl_up_sync(0xffffffffu, v, 1); return tx == 0 ? zero : r; };
+    auto from_right = [&](T v) { const T r = __shfl_down_sync(0xffffffffu, v, 1); return tx == TX - 1 ? zero : r; };
+
+    int zl = wrapz(z0 - 1), zt = wrapz(z0 - 2);         // this plane / the plane the gathered density belongs to
+    unsigned lk = 0;
+    if (HAS_SOLID) lk = __ldg(links + (long long)zl * pl + own_xy);
+
+#pragma unroll 1
+    for (int it = 0; it < niter; ++it) {
+        const long long n = (long long)zl * pl + own_xy;
+        const bool store_h = it >= 1 && it <= niter - 2;
+        const bool store_rho = it >= 2;                 // target plane z-1 lies in [z0, z1)
+        const int s0 = (it + 1) & 3;                    // ring slot of plane z
+        const bool fluid = !HAS_SOLID || !(lk & OP_SOLID_BIT);   // nothing happens inside a particle
+        T* SU = SUb + (it & 1) * 12 * SUP;
+
+        // ---- pull: the stage holds h_i(x - c_i) for the whole tile (Eq. 5, periodic) ----
+        mbar_wait(full, it & 1);
+        if (wrap_tile) mbar_wait(patch, it & 1);
+        T fr[Q], fb[Q];
+#pragma unroll
+        for (int i = 0; i < Q; ++i) {
+            fr[i] = stage[L::slot_off(i) + L::read_off(i, tx, ty)];
+            fb[i] = stage[L::slot_off(Q + i) + L::read_off(i, tx, ty)];
+        }
+        if (HAS_SOLID && (lk & 0x7FFFEu)) {             // halfway bounce-back (Eq. 23-24, u_b = 0): f_i(x) = h_opp(i)(x) when x - c_i is solid
+#pragma unroll
+            for (int i = 1; i < Q; ++i)
+                if (lk >> dir_opp(i) & 1u) {
+                    fr[i] = __ldg(h + (long long)dir_opp(i) * NP + n);
+                    fb[i] = __ldg(h + (long long)(Q + dir_opp(i)) * NP + n);
+                }
+        }
+        __syncwarp();
+        if (tx == 0) mbar_arrive(done);                 // the producer may refill the stage with the next plane
+
+        // ---- moments (Eq. 6-7), common velocity (S4), Shan-Chen force (S2, S3, S6, S7) ----
+        T rr = zero, rb = zero, ux = zero, uy = zero, uz = zero;
+        T er[3] = {zero, zero, zero}, eb[3] = {zero, zero, zero};
+        if (fluid) {
+            T jr[3], jb[3];
+            moments19<T>(fr, rr, jr[0], jr[1], jr[2]);
+            moments19<T>(fb, rb, jb[0], jb[1], jb[2]);
+            T gr[3] = {zero, zero, zero}, gb[3] = {zero, zero, zero};
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
+                const int op = own_r + pair_cy(p) * RW + pair_cx(p), om = own_r - pair_cy(p) * RW - pair_cx(p);
+                T bp = ring[(sp * 2 + 1) * RS + op], bm = ring[(sm_ * 2 + 1) * RS + om];
+                T rp = ring[(sp * 2 + 0) * RS + op], rm = ring[(sm_ * 2 + 0) * RS + om];
+                if (HAS_SOLID) {                                           // a solid neighbour counts psi = 0 (S7)
+                    if (lk >> (2 * p + 1) & 1u) { bp = zero; rp = zero; }
+                    if (lk >> (2 * p + 2) & 1u) { bm = zero; rm = zero; }
+                }
+                const T db = w_pair<T>(p) * (bp - bm);
+                const T dr = w_pair<T>(p) * (rp - rm);
+                if (pair_cx(p)) { gr[0] += T(pair_cx(p)) * db; gb[0] += T(pair_cx(p)) * dr; }
+                if (pair_cy(p)) { gr[1] += T(pair_cy(p)) * db; gb[1] += T(pair_cy(p)) * dr; }
+                if (pair_cz(p)) { gr[2] += T(pair_cz(p)) * db; gb[2] += T(pair_cz(p)) * dr; }
+            }
+            const T den = om_r * rr + om_b * rb;
+            const T inv = den != zero ? T(1) / den : zero;
+            ux = (om_r * jr[0] + om_b * jb[0]) * inv;
+            uy = (om_r * jr[1] + om_b * jb[1]) * inv;
+            uz = (om_r * jr[2] + om_b * jb[2]) * inv;
+            er[0] = ux - G * gr[0]; er[1] = uy - G * gr[1]; er[2] = uz - G * gr[2];
+            eb[0] = ux - G * gb[0]; eb[1] = uy - G * gb[1]; eb[2] = uz - G * gb[2];
+            // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5); aligned stores ----
+            collide19<T>(fr, rr, T(1) - om_r, ux, uy, uz, er[0], er[1], er[2]);
+            collide19<T>(fb, rb, T(1) - om_b, ux, uy, uz, eb[0], eb[1], eb[2]);
+            if (store_h) {
+                T* o = g + n;
+#pragma unroll
+                for (int i = 0; i < Q; ++i) {
+                    o[(long long)i * NP] = fr[i];
+                    o[(long long)(Q + i) * NP] = fb[i];
+                }
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < Q; ++i) { fr[i] = zero; fb[i] = zero; }
+        }
+
+        // ---- density gather, x stage (warp shuffles) and publication of the y-stage inputs ----
+        T u0[2][3], ee[2][3];                            // U0[dz] row sums; on lanes tx = 0 / TX-1: what leaves the tile in x with c_y = 0
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            T (&hk)[Q] = k == 0 ? fr : fb;
+            T up[3] = {zero, zero, zero}, um[3] = {zero, zero, zero};
+            T* sup0 = SU + (k * 6 + 1) * SUP;            // Up[dz = 0]
+            T* sum0 = SU + (k * 6 + 4) * SUP;            // Um[dz = 0]
+            u0[k][0] = zero; u0[k][1] = hk[0]; u0[k][2] = zero;
+            ee[k][0] = ee[k][1] = ee[k][2] = zero;
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                const T h1 = hk[2 * p + 1], h2 = hk[2 * p + 2];
+                T l = zero, r = zero;
+                if (p == 0 || (p >= 3 && p <= 6)) { l = from_left(h1); r = from_right(h2); }
+                if (p == 0) {                                              // +x / -x
+                    u0[k][1] += l; u0[k][1] += r;
+                    if (tx == TX - 1) ee[k][1] = h1;
+                    if (tx == 0) ee[k][1] = h2;
+                } else if (p == 1) { up[1] = h1; um[1] = h2; }              // +y / -y
+                else if (p == 2) { u0[k][2] = h1; u0[k][0] = h2; }          // +z / -z
+                else if (p == 3) {                                         // +x+y / -x-y
+                    up[1] += l; um[1] += r;
+                    if (tx == TX - 1) sup0[own_s + 1] = h1;
+                    if (tx == 0) sum0[own_s - 1] = h2;
+                } else if (p == 4) {                                       // +x-y / -x+y
+                    um[1] += l; up[1] += r;
+                    if (tx == TX - 1) sum0[own_s + 1] = h1;
+                    if (tx == 0) sup0[own_s - 1] = h2;
+                } else if (p == 5) {                                       // +x+z / -x-z
+                    u0[k][2] += l; u0[k][0] += r;
+                    if (tx == TX - 1) ee[k][2] = h1;
+                    if (tx == 0) ee[k][0] = h2;
+                } else if (p == 6) {                                       // +x-z / -x+z
+                    u0[k][0] += l; u0[k][2] += r;
+                    if (tx == TX - 1) ee[k][0] = h1;
+                    if (tx == 0) ee[k][2] = h2;
+                } else if (p == 7) { up[2] = h1; um[0] = h2; }              // +y+z / -y-z
+                else { up[0] = h1; um[2] = h2; }                           // +y-z / -y+z
+                // corners: only c_z = 0 directions reach a diagonal tile, so the target plane is this plane
+                if (store_h && (p == 3 || p == 4)) {
+                    if (p == 3 && tx == TX - 1 && ty == TY - 1) ro.xy[k * ro.s_xy + zl * psxy + (btyp * ntx + btxp) * 4 + 0] = h1;
+                    if (p == 3 && tx == 0 && ty == 0) ro.xy[k * ro.s_xy + zl * psxy + (btym * ntx + btxm) * 4 + 3] = h2;
+                    if (p == 4 && tx == TX - 1 && ty == 0) ro.xy[k * ro.s_xy + zl * psxy + (btym * ntx + btxp) * 4 + 2] = h1;
+                    if (p == 4 && tx == 0 && ty == TY - 1) ro.xy[k * ro.s_xy + zl * psxy + (btyp * ntx + btxm) * 4 + 1] = h2;
+                }
+            }
+            if (HAS_SOLID && fluid && (lk & 0x7FFFEu)) {                   // bounced-back arrivals of the next step come from this node
+                T bs = zero;
+#pragma unroll
+                for (int i = 1; i < Q; ++i)
+                    if (lk >> i & 1u) bs += hk[i];
+                u0[k][1] += bs;
+            }
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                SU[(k * 6 + d) * SUP + own_s] = up[d];
+                SU[(k * 6 + 3 + d) * SUP + own_s] = um[d];
+            }
+            if (ty == 0 || ty == TY - 1) {                                 // the row beyond the tile edge receives exactly Um (Up)
+                const bool lo = ty == 0;
+                const T a_m = lo ? um[0] : up[0], a_0 = lo ? um[1] : up[1], a_p = lo ? um[2] : up[2];
+                const T out = row_acc[k][0] + a_m;
+                row_acc[k][0] = row_acc[k][1] + a_0;
+                row_acc[k][1] = a_p;
+                if (store_rho) ro.y[k * ro.s_y + zt * psy + ((lo ? btym : btyp) * 2 + (lo ? 1 : 0)) * nx + x] = out;
+            }
+        }
+        if (it <= niter - 2) ring_store((it + 3) & 3);                     // rho(t) of plane z+2, loaded one iteration ago
+
+        named_barrier<1, NT>();
+
+        // ---- y stage and z pipeline of the gather; exports across the tile's x edges ----
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            T a[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                a[d] = u0[k][d];
+                if (ty > 0) a[d] += SU[(k * 6 + d) * SUP + own_s - RW];            // Up[dz](y-1)
+                if (ty < TY - 1) a[d] += SU[(k * 6 + 3 + d) * SUP + own_s + RW];   // Um[dz](y+1)
+            }
+            const T out = own_acc[k][0] + a[0];
+            own_acc[k][0] = own_acc[k][1] + a[1];
+            own_acc[k][1] = a[2];
+            if (store_rho) ro.in[k * ro.s_in + (long long)zt * pl + own_xy] = out;
+            if (tx == 0 || tx == TX - 1) {
+                const bool lo = tx == 0;
+                const int vc = lo ? own_s - 1 : own_s + 1;                 // the virtual column next to this lane
+                T a_0 = ee[k][1];
+                if (ty > 0) a_0 += SU[(k * 6 + 1) * SUP + vc - RW];
+                if (ty < TY - 1) a_0 += SU[(k * 6 + 4) * SUP + vc + RW];
+                const T hout = col_acc[k][0] + ee[k][0];
+                col_acc[k][0] = col_acc[k][1] + a_0;
+                col_acc[k][1] = ee[k][2];
+                if (store_rho) ro.x[k * ro.s_x + zt * psx + ((bty * ntx + (lo ? btxm : btxp)) * 2 + (lo ? 1 : 0)) * TY + ty] = hout;
+            }
+        }
+        if (it <= niter - 3) ring_load(z0 + 2 + it);                       // plane z+3
+        zt = zl;
+        zl = zl + 1 == nz ? 0 : zl + 1;
+        if (HAS_SOLID && it + 1 < niter) lk = __ldg(links + (long long)zl * pl + own_xy);
+    }
+}
+
+}  // namespace lb

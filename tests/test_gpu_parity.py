@@ -12,8 +12,8 @@ from paper_2112_08264_b200 import workloads as w
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [B.LB_KERNEL_TWOPASS, B.LB_KERNEL_ONEPASS]
-KNAME = {B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass"}
+KERNELS = [B.LB_KERNEL_TWOPASS, B.LB_KERNEL_ONEPASS, B.LB_KERNEL_TMA]
+KNAME = {B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass", B.LB_KERNEL_TMA: "tma"}
 
 
 @pytest.fixture(scope="module", autouse=True)
