@@ -553,7 +553,7 @@ int launch_tma(lb_ctx* c) {
     }
     const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc - 1) / c->zc);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    kern<<<grid, OP_TX * OP_TY + 32, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], static_cast<const T*>(c->f[c->cur]),
+    kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], static_cast<const T*>(c->f[c->cur]),
                                                         static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                         rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
                                                         c->zc, om_r, om_b, G);

@@ -76,9 +76,11 @@ struct TmaLayout {
     static constexpr unsigned STAGE_TX_BYTES = unsigned(2 * (9 * NT + 10 * W * TY) * sizeof(T));   // bytes the 38 boxes deliver
     static constexpr int RING = STAGE + STAGE_ELEMS;                   // [4][2][RS]      rho(t), planes z-1..z+2
     static constexpr int SU = RING + 8 * RS;                           // [2][2][6][SUP]  double-buffered Up[dz], Um[dz] per component
-    static constexpr int END = SU + 24 * SUP;
+    static constexpr int XM = SU + 24 * SUP;                           // [2][NT][4]      rho^k, j^k of every node, exchanged between the two components' threads
+    static constexpr int RP = XM + 8 * NT;                             // [8][2*NT]       thread-private landing slots of the ring pieces (cp.async)
+    static constexpr int END = RP + 16 * NT;
     static constexpr size_t BAR_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
-    static constexpr size_t BYTES = BAR_BYTE_OFF + 4 * sizeof(unsigned long long);
+    static constexpr size_t BYTES = BAR_BYTE_OFF + 8 * sizeof(unsigned long long);
     // where consumer (tx, ty) finds f_i = h_i(x - c_i) inside slot i
     __host__ __device__ static constexpr int read_off(int i, int tx, int ty) {
         return dir_cx(i) == 0 ? ty * TX + tx : ty * W + tx + (dir_cx(i) > 0 ? PADX - 1 : 1);
@@ -87,24 +89,34 @@ struct TmaLayout {
 
 
 // ---- the kernel ------------------------------------------------------------------------------------------
+// Threads: 2*NT consumers (component k = t / NT, node (tx, ty) = ((t % NT) % 32, (t % NT) / 32): one warp per
+// tile row and component) followed by one producer warp group (only its first warp works).  The producer
+// group gives its registers to the consumers (setmaxnreg), which is why it is a whole warp group.
 template <typename T, bool HAS_SOLID, int TY>
-__global__ void __launch_bounds__(32 * TY + 32, 1)
+__global__ void __launch_bounds__(2 * 32 * TY + 128, 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
            const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
            T om_r, T om_b, T G) {
     using L = TmaLayout<T, TY>;
-    constexpr int TX = L::TX, NT = L::NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
+    constexpr int TX = L::TX, NT = L::NT, NC = 2 * NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     static_assert(RS <= 2 * NT, "ring fill: at most two positions per consumer thread");
+    static_assert(TY >= 2 && TY <= 8, "one named barrier per tile row (ids 1..TY)");
+    // register hand-over between the warp groups: (2*NT + 128) threads start with 65536 / threads registers each
+    constexpr int START_REGS = (65536 / (NC + 128)) / 8 * 8;
+    constexpr int PRODUCER_REGS = 32;
+    constexpr int CONSUMER_REGS = (START_REGS + (START_REGS - PRODUCER_REGS) * 128 / NC) / 8 * 8;
     extern __shared__ __align__(1024) unsigned char smem_tma[];
     T* sm = reinterpret_cast<T*>(smem_tma);
     T* stage = sm + L::STAGE;
     T* ring = sm + L::RING;
     T* SUb = sm + L::SU;
+    T* xm = sm + L::XM;
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma + L::BAR_BYTE_OFF);
     unsigned long long* full = bars;          // the 38 boxes of the next plane have landed (tx bytes)
     unsigned long long* patch = bars + 1;     // ... and the producer has patched the wrapped column / row (boundary tiles)
-    unsigned long long* done = bars + 2;      // every consumer warp has copied the stage into registers
+    unsigned long long* done = bars + 2;      // every consumer warp has copied its part of the stage into registers
+    unsigned long long* pub = bars + 3;       // every consumer warp has published its y-stage inputs of this plane
 
     const int t = threadIdx.x;
     const int ntx = nx / TX, nty = ny / TY;
@@ -120,14 +132,17 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     if (t == 0) {
         mbar_init(full, 1);
         mbar_init(patch, 1);
-        mbar_init(done, TY);
+        mbar_init(done, 2 * TY);
+        mbar_init(pub, 2 * TY);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
     // =================================== producer warp ===================================
-    if (t >= NT) {
-        const int lane = t - NT;
+    if (t >= NC) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PRODUCER_REGS));
+        if (t >= NC + 32) return;
+        const int lane = t - NC;
         for (int j = 0; j < niter; ++j) {
             const int z = z0 - 1 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
@@ -181,7 +196,10 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     }
 
     // =================================== consumers ===================================
-    const int tx = t % TX, ty = t / TX;
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(CONSUMER_REGS));
+    const int k = t / NT;                                                  // component of this thread (warp-uniform)
+    const int tl = t - k * NT;
+    const int tx = tl % TX, ty = tl / TX;
     const int x = x0 + tx, y = y0 + ty;
     const int own_xy = y * nx + x;
     const int own_r = (ty + 1) * RW + tx + 1;                              // ring position (tile + frame)
@@ -190,13 +208,24 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const int btxm = btx == 0 ? ntx - 1 : btx - 1, btxp = btx == ntx - 1 ? 0 : btx + 1;
     const int btym = bty == 0 ? nty - 1 : bty - 1, btyp = bty == nty - 1 ? 0 : bty + 1;
     const T zero = T(0);
+    const T omc = T(1) - (k == 0 ? om_r : om_b);
+    const T* stage_k = stage + k * (9 * L::NA + 10 * L::WA);
+    const T* hk = h + (long long)k * Q * NP;
+    T* gk = g + (long long)k * Q * NP + own_xy;
+    const T* ring_o = ring + (1 - k) * RS;                                 // the OTHER component's density (S2)
+    T* SUk = SUb + k * 6 * SUP;
+    T* ro_in = ro.in + k * ro.s_in + own_xy;
+    T* ro_x = ro.x + k * ro.s_x;
+    T* ro_y = ro.y + k * ro.s_y;
+    T* ro_xy = ro.xy + k * ro.s_xy;
+    const bool lane_lo = tx == 0, lane_hi = tx == TX - 1, row_lo = ty == 0, row_hi = ty == TY - 1;
 
-    // ---- density ring: every consumer owns ring positions t and t + NT and assembles them from the four
-    //      single-writer arrays in the fixed order ((in + x) + y) + xy ----
+    // ---- density ring: every consumer owns ring positions tl and tl + NT of its component and assembles them
+    //      from the four single-writer arrays in the fixed order ((in + x) + y) + xy ----
     int o_in[2], o_x[2], o_y[2], o_xy[2];
 #pragma unroll
     for (int a = 0; a < 2; ++a) {
-        const int pos = t + a * NT;
+        const int pos = tl + a * NT;
         o_in[a] = o_x[a] = o_y[a] = o_xy[a] = -1;
         if (pos < RS) {
             const int rx = pos % RW - 1, ry = pos / RW - 1;
@@ -209,52 +238,48 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             if (ex && ey) o_xy[a] = (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
         }
     }
-    T raw[2][2][4];                                                        // [position][component][in, x, y, xy] of the plane in flight
-    auto ring_load = [&](int p) {
-        const long long zl = wrapz(p);
+    const T* ri_in = ri.in + k * ri.s_in;
+    const T* ri_x = ri.x + k * ri.s_x;
+    const T* ri_y = ri.y + k * ri.s_y;
+    const T* ri_xy = ri.xy + k * ri.s_xy;
+    T* rp = sm + L::RP + t;                                                // [position*4 + piece][2*NT]: this thread's landing slots
+    auto ring_load = [&](int p) {                                          // asynchronous: no registers in flight
+        const long long zp = wrapz(p);
 #pragma unroll
-        for (int a = 0; a < 2; ++a)
-#pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                if (o_in[a] >= 0) raw[a][k][0] = __ldg(ri.in + k * ri.s_in + zl * pl + o_in[a]);
-                if (o_x[a] >= 0) raw[a][k][1] = __ldg(ri.x + k * ri.s_x + zl * psx + o_x[a]);
-                if (o_y[a] >= 0) raw[a][k][2] = __ldg(ri.y + k * ri.s_y + zl * psy + o_y[a]);
-                if (o_xy[a] >= 0) raw[a][k][3] = __ldg(ri.xy + k * ri.s_xy + zl * psxy + o_xy[a]);
-            }
+        for (int a = 0; a < 2; ++a) {
+            if (o_in[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 0) * NC, ri_in + zp * pl + o_in[a]);
+            if (o_x[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 1) * NC, ri_x + zp * psx + o_x[a]);
+            if (o_y[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 2) * NC, ri_y + zp * psy + o_y[a]);
+            if (o_xy[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 3) * NC, ri_xy + zp * psxy + o_xy[a]);
+        }
+        cp_async_commit();
     };
-    auto ring_store = [&](int slot) {
+    auto ring_store = [&](int slot) {                                      // the same thread reads what it asked for: no barrier
+        cp_async_wait<0>();
 #pragma unroll
-        for (int a = 0; a < 2; ++a)
-#pragma unroll
-            for (int k = 0; k < 2; ++k) {
-                if (o_in[a] < 0) continue;
-                T v = raw[a][k][0];
-                if (o_x[a] >= 0) v += raw[a][k][1];
-                if (o_y[a] >= 0) v += raw[a][k][2];
-                if (o_xy[a] >= 0) v += raw[a][k][3];
-                ring[(slot * 2 + k) * RS + t + a * NT] = v;
-            }
+        for (int a = 0; a < 2; ++a) {
+            if (o_in[a] < 0) continue;
+            T v = rp[(a * 4 + 0) * NC];
+            if (o_x[a] >= 0) v += rp[(a * 4 + 1) * NC];
+            if (o_y[a] >= 0) v += rp[(a * 4 + 2) * NC];
+            if (o_xy[a] >= 0) v += rp[(a * 4 + 3) * NC];
+            ring[(slot * 2 + k) * RS + tl + a * NT] = v;
+        }
     };
-#pragma unroll
-    for (int a = 0; a < 2; ++a)
-#pragma unroll
-        for (int k = 0; k < 2; ++k)
-#pragma unroll
-            for (int c = 0; c < 4; ++c) raw[a][k][c] = zero;
 #pragma unroll 1
     for (int p = 0; p < 3; ++p) {                                          // planes z0-2, z0-1, z0 -> slots 0, 1, 2
         ring_load(z0 - 2 + p);
         ring_store(p);
     }
     ring_load(z0 + 1);                                                     // stored in iteration 0
-    named_barrier<1, NT>();
+    named_barrier<TY + 1, NC>();
 
     // ---- per-thread state carried along z ----
-    T own_acc[2][2] = {{zero, zero}, {zero, zero}};     // z pipeline of this node's gathered density: [k][0] = A_+1(z-2) + A_0(z-1), [k][1] = A_+1(z-1)
-    T row_acc[2][2] = {{zero, zero}, {zero, zero}};     // the same for the export across the tile's y edge (warps ty = 0 and TY-1)
-    T col_acc[2][2] = {{zero, zero}, {zero, zero}};     // ... across the tile's x edge (lanes tx = 0 and TX-1)
-    auto from_left = [&](T v) { const T r = __shfl_up_sync(0xffffffffu, v, 1); return tx == 0 ? zero : r; };
-    auto from_right = [&](T v) { const T r = __shfl_down_sync(0xffffffffu, v, 1); return tx == TX - 1 ? zero : r; };
+    T own_acc[2] = {zero, zero};     // z pipeline of this node's gathered density: [0] = A_+1(z-2) + A_0(z-1), [1] = A_+1(z-1)
+    T row_acc[2] = {zero, zero};     // the same for the export across the tile's y edge (warps ty = 0 and TY-1)
+    T col_acc[2] = {zero, zero};     // ... across the tile's x edge (lanes tx = 0 and TX-1)
+    auto from_left = [&](T v) { const T r = __shfl_up_sync(0xffffffffu, v, 1); return lane_lo ? zero : r; };
+    auto from_right = [&](T v) { const T r = __shfl_down_sync(0xffffffffu, v, 1); return lane_hi ? zero : r; };
 
     int zl = wrapz(z0 - 1), zt = wrapz(z0 - 2);         // this plane / the plane the gathered density belongs to
     unsigned lk = 0;
@@ -262,176 +287,171 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
 
 #pragma unroll 1
     for (int it = 0; it < niter; ++it) {
-        const long long n = (long long)zl * pl + own_xy;
+        const long long zoff = (long long)zl * pl;
         const bool store_h = it >= 1 && it <= niter - 2;
         const bool store_rho = it >= 2;                 // target plane z-1 lies in [z0, z1)
         const int s0 = (it + 1) & 3;                    // ring slot of plane z
         const bool fluid = !HAS_SOLID || !(lk & OP_SOLID_BIT);   // nothing happens inside a particle
-        T* SU = SUb + (it & 1) * 12 * SUP;
+        T* SU = SUk + (it & 1) * 12 * SUP;
 
         // ---- pull: the stage holds h_i(x - c_i) for the whole tile (Eq. 5, periodic) ----
         mbar_wait(full, it & 1);
         if (wrap_tile) mbar_wait(patch, it & 1);
-        T fr[Q], fb[Q];
+        T f[Q];
 #pragma unroll
-        for (int i = 0; i < Q; ++i) {
-            fr[i] = stage[L::slot_off(i) + L::read_off(i, tx, ty)];
-            fb[i] = stage[L::slot_off(Q + i) + L::read_off(i, tx, ty)];
-        }
+        for (int i = 0; i < Q; ++i) f[i] = stage_k[L::slot_off(i) + L::read_off(i, tx, ty)];
         if (HAS_SOLID && (lk & 0x7FFFEu)) {             // halfway bounce-back (Eq. 23-24, u_b = 0): f_i(x) = h_opp(i)(x) when x - c_i is solid
 #pragma unroll
             for (int i = 1; i < Q; ++i)
-                if (lk >> dir_opp(i) & 1u) {
-                    fr[i] = __ldg(h + (long long)dir_opp(i) * NP + n);
-                    fb[i] = __ldg(h + (long long)(Q + dir_opp(i)) * NP + n);
-                }
+                if (lk >> dir_opp(i) & 1u) f[i] = __ldg(hk + (long long)dir_opp(i) * NP + zoff + own_xy);
         }
         __syncwarp();
-        if (tx == 0) mbar_arrive(done);                 // the producer may refill the stage with the next plane
+        if (lane_lo) mbar_arrive(done);                 // the producer may refill the stage with the next plane
 
-        // ---- moments (Eq. 6-7), common velocity (S4), Shan-Chen force (S2, S3, S6, S7) ----
-        T rr = zero, rb = zero, ux = zero, uy = zero, uz = zero;
-        T er[3] = {zero, zero, zero}, eb[3] = {zero, zero, zero};
+        // ---- moments of this component (Eq. 6-7), exchanged with the other component's thread of the same node ----
+        T rho = zero, jx = zero, jy = zero, jz = zero;
+        if (fluid) moments19<T>(f, rho, jx, jy, jz);
+        else {
+#pragma unroll
+            for (int i = 0; i < Q; ++i) f[i] = zero;
+        }
+        {
+            T* mine = xm + (k * NT + tl) * 4;
+            mine[0] = rho; mine[1] = jx; mine[2] = jy; mine[3] = jz;
+        }
+        asm volatile("bar.sync %0, 64;" ::"r"(ty + 1) : "memory");         // the two warps (red, blue) of this tile row
+        T ux = zero, uy = zero, uz = zero, ex = zero, ey = zero, ez = zero;
         if (fluid) {
-            T jr[3], jb[3];
-            moments19<T>(fr, rr, jr[0], jr[1], jr[2]);
-            moments19<T>(fb, rb, jb[0], jb[1], jb[2]);
-            T gr[3] = {zero, zero, zero}, gb[3] = {zero, zero, zero};
+            const T* other = xm + ((1 - k) * NT + tl) * 4;
+            const T orho = other[0], ojx = other[1], ojy = other[2], ojz = other[3];
+            const T rr = k == 0 ? rho : orho, rb = k == 0 ? orho : rho;
+            const T jrx = k == 0 ? jx : ojx, jry = k == 0 ? jy : ojy, jrz = k == 0 ? jz : ojz;
+            const T jbx = k == 0 ? ojx : jx, jby = k == 0 ? ojy : jy, jbz = k == 0 ? ojz : jz;
+            const T den = om_r * rr + om_b * rb;                            // common velocity (S4)
+            const T inv = den != zero ? T(1) / den : zero;
+            ux = (om_r * jrx + om_b * jbx) * inv;
+            uy = (om_r * jry + om_b * jby) * inv;
+            uz = (om_r * jrz + om_b * jbz) * inv;
+            // du^k = -G sum_i w_i rho^kbar(x+c_i) c_i (S2, S3, S6); a solid neighbour counts psi = 0 (S7)
+            T gx = zero, gy = zero, gz = zero;
 #pragma unroll
             for (int p = 0; p < 9; ++p) {
                 const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
-                const int op = own_r + pair_cy(p) * RW + pair_cx(p), om = own_r - pair_cy(p) * RW - pair_cx(p);
-                T bp = ring[(sp * 2 + 1) * RS + op], bm = ring[(sm_ * 2 + 1) * RS + om];
-                T rp = ring[(sp * 2 + 0) * RS + op], rm = ring[(sm_ * 2 + 0) * RS + om];
-                if (HAS_SOLID) {                                           // a solid neighbour counts psi = 0 (S7)
-                    if (lk >> (2 * p + 1) & 1u) { bp = zero; rp = zero; }
-                    if (lk >> (2 * p + 2) & 1u) { bm = zero; rm = zero; }
+                T vp = ring_o[sp * 2 * RS + own_r + pair_cy(p) * RW + pair_cx(p)];
+                T vm = ring_o[sm_ * 2 * RS + own_r - pair_cy(p) * RW - pair_cx(p)];
+                if (HAS_SOLID) {
+                    if (lk >> (2 * p + 1) & 1u) vp = zero;
+                    if (lk >> (2 * p + 2) & 1u) vm = zero;
                 }
-                const T db = w_pair<T>(p) * (bp - bm);
-                const T dr = w_pair<T>(p) * (rp - rm);
-                if (pair_cx(p)) { gr[0] += T(pair_cx(p)) * db; gb[0] += T(pair_cx(p)) * dr; }
-                if (pair_cy(p)) { gr[1] += T(pair_cy(p)) * db; gb[1] += T(pair_cy(p)) * dr; }
-                if (pair_cz(p)) { gr[2] += T(pair_cz(p)) * db; gb[2] += T(pair_cz(p)) * dr; }
+                const T d = w_pair<T>(p) * (vp - vm);
+                if (pair_cx(p)) gx += T(pair_cx(p)) * d;
+                if (pair_cy(p)) gy += T(pair_cy(p)) * d;
+                if (pair_cz(p)) gz += T(pair_cz(p)) * d;
             }
-            const T den = om_r * rr + om_b * rb;
-            const T inv = den != zero ? T(1) / den : zero;
-            ux = (om_r * jr[0] + om_b * jb[0]) * inv;
-            uy = (om_r * jr[1] + om_b * jb[1]) * inv;
-            uz = (om_r * jr[2] + om_b * jb[2]) * inv;
-            er[0] = ux - G * gr[0]; er[1] = uy - G * gr[1]; er[2] = uz - G * gr[2];
-            eb[0] = ux - G * gb[0]; eb[1] = uy - G * gb[1]; eb[2] = uz - G * gb[2];
-            // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5); aligned stores ----
-            collide19<T>(fr, rr, T(1) - om_r, ux, uy, uz, er[0], er[1], er[2]);
-            collide19<T>(fb, rb, T(1) - om_b, ux, uy, uz, eb[0], eb[1], eb[2]);
-            if (store_h) {
-                T* o = g + n;
-#pragma unroll
-                for (int i = 0; i < Q; ++i) {
-                    o[(long long)i * NP] = fr[i];
-                    o[(long long)(Q + i) * NP] = fb[i];
-                }
-            }
-        } else {
-#pragma unroll
-            for (int i = 0; i < Q; ++i) { fr[i] = zero; fb[i] = zero; }
+            ex = ux - G * gx; ey = uy - G * gy; ez = uz - G * gz;
+            // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) ----
+            collide19<T>(f, rho, omc, ux, uy, uz, ex, ey, ez);
         }
 
         // ---- density gather, x stage (warp shuffles) and publication of the y-stage inputs ----
-        T u0[2][3], ee[2][3];                            // U0[dz] row sums; on lanes tx = 0 / TX-1: what leaves the tile in x with c_y = 0
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
-            T (&hk)[Q] = k == 0 ? fr : fb;
-            T up[3] = {zero, zero, zero}, um[3] = {zero, zero, zero};
-            T* sup0 = SU + (k * 6 + 1) * SUP;            // Up[dz = 0]
-            T* sum0 = SU + (k * 6 + 4) * SUP;            // Um[dz = 0]
-            u0[k][0] = zero; u0[k][1] = hk[0]; u0[k][2] = zero;
-            ee[k][0] = ee[k][1] = ee[k][2] = zero;
+        T u0[3] = {zero, f[0], zero};                    // U0[dz] row sums
+        T ee[3] = {zero, zero, zero};                    // on lanes tx = 0 / TX-1: what leaves the tile in x with c_y = 0
+        T up[3] = {zero, zero, zero}, um[3] = {zero, zero, zero};
+        {
+            T* sup0 = SU + 1 * SUP;                      // Up[dz = 0]
+            T* sum0 = SU + 4 * SUP;                      // Um[dz = 0]
 #pragma unroll
             for (int p = 0; p < 9; ++p) {
-                const T h1 = hk[2 * p + 1], h2 = hk[2 * p + 2];
+                const T h1 = f[2 * p + 1], h2 = f[2 * p + 2];
                 T l = zero, r = zero;
                 if (p == 0 || (p >= 3 && p <= 6)) { l = from_left(h1); r = from_right(h2); }
                 if (p == 0) {                                              // +x / -x
-                    u0[k][1] += l; u0[k][1] += r;
-                    if (tx == TX - 1) ee[k][1] = h1;
-                    if (tx == 0) ee[k][1] = h2;
+                    u0[1] += l; u0[1] += r;
+                    ee[1] = lane_hi ? h1 : h2;
                 } else if (p == 1) { up[1] = h1; um[1] = h2; }              // +y / -y
-                else if (p == 2) { u0[k][2] = h1; u0[k][0] = h2; }          // +z / -z
+                else if (p == 2) { u0[2] = h1; u0[0] = h2; }                // +z / -z
                 else if (p == 3) {                                         // +x+y / -x-y
                     up[1] += l; um[1] += r;
-                    if (tx == TX - 1) sup0[own_s + 1] = h1;
-                    if (tx == 0) sum0[own_s - 1] = h2;
+                    if (lane_hi) sup0[own_s + 1] = h1;
+                    if (lane_lo) sum0[own_s - 1] = h2;
                 } else if (p == 4) {                                       // +x-y / -x+y
                     um[1] += l; up[1] += r;
-                    if (tx == TX - 1) sum0[own_s + 1] = h1;
-                    if (tx == 0) sup0[own_s - 1] = h2;
+                    if (lane_hi) sum0[own_s + 1] = h1;
+                    if (lane_lo) sup0[own_s - 1] = h2;
                 } else if (p == 5) {                                       // +x+z / -x-z
-                    u0[k][2] += l; u0[k][0] += r;
-                    if (tx == TX - 1) ee[k][2] = h1;
-                    if (tx == 0) ee[k][0] = h2;
+                    u0[2] += l; u0[0] += r;
+                    if (lane_hi) ee[2] = h1;
+                    if (lane_lo) ee[0] = h2;
                 } else if (p == 6) {                                       // +x-z / -x+z
-                    u0[k][0] += l; u0[k][2] += r;
-                    if (tx == TX - 1) ee[k][0] = h1;
-                    if (tx == 0) ee[k][2] = h2;
+                    u0[0] += l; u0[2] += r;
+                    if (lane_hi) ee[0] = h1;
+                    if (lane_lo) ee[2] = h2;
                 } else if (p == 7) { up[2] = h1; um[0] = h2; }              // +y+z / -y-z
                 else { up[0] = h1; um[2] = h2; }                           // +y-z / -y+z
-                // corners: only c_z = 0 directions reach a diagonal tile, so the target plane is this plane
-                if (store_h && (p == 3 || p == 4)) {
-                    if (p == 3 && tx == TX - 1 && ty == TY - 1) ro.xy[k * ro.s_xy + zl * psxy + (btyp * ntx + btxp) * 4 + 0] = h1;
-                    if (p == 3 && tx == 0 && ty == 0) ro.xy[k * ro.s_xy + zl * psxy + (btym * ntx + btxm) * 4 + 3] = h2;
-                    if (p == 4 && tx == TX - 1 && ty == 0) ro.xy[k * ro.s_xy + zl * psxy + (btym * ntx + btxp) * 4 + 2] = h1;
-                    if (p == 4 && tx == 0 && ty == TY - 1) ro.xy[k * ro.s_xy + zl * psxy + (btyp * ntx + btxm) * 4 + 1] = h2;
-                }
             }
             if (HAS_SOLID && fluid && (lk & 0x7FFFEu)) {                   // bounced-back arrivals of the next step come from this node
                 T bs = zero;
 #pragma unroll
                 for (int i = 1; i < Q; ++i)
-                    if (lk >> i & 1u) bs += hk[i];
-                u0[k][1] += bs;
+                    if (lk >> i & 1u) bs += f[i];
+                u0[1] += bs;
             }
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                SU[(k * 6 + d) * SUP + own_s] = up[d];
-                SU[(k * 6 + 3 + d) * SUP + own_s] = um[d];
-            }
-            if (ty == 0 || ty == TY - 1) {                                 // the row beyond the tile edge receives exactly Um (Up)
-                const bool lo = ty == 0;
-                const T a_m = lo ? um[0] : up[0], a_0 = lo ? um[1] : up[1], a_p = lo ? um[2] : up[2];
-                const T out = row_acc[k][0] + a_m;
-                row_acc[k][0] = row_acc[k][1] + a_0;
-                row_acc[k][1] = a_p;
-                if (store_rho) ro.y[k * ro.s_y + zt * psy + ((lo ? btym : btyp) * 2 + (lo ? 1 : 0)) * nx + x] = out;
+                SU[d * SUP + own_s] = up[d];
+                SU[(3 + d) * SUP + own_s] = um[d];
             }
         }
         if (it <= niter - 2) ring_store((it + 3) & 3);                     // rho(t) of plane z+2, loaded one iteration ago
+        __syncwarp();
+        if (lane_lo) mbar_arrive(pub);
 
-        named_barrier<1, NT>();
+        // ---- global stores that need nothing from the other warps: h, the y-edge and corner exports ----
+        if (fluid && store_h) {
+            T* o = gk + zoff;
+#pragma unroll
+            for (int i = 0; i < Q; ++i) o[(long long)i * NP] = f[i];
+        }
+        if (row_lo || row_hi) {                                            // the row beyond the tile edge receives exactly Um (Up)
+            const T a_m = row_lo ? um[0] : up[0], a_0 = row_lo ? um[1] : up[1], a_p = row_lo ? um[2] : up[2];
+            const T out = row_acc[0] + a_m;
+            row_acc[0] = row_acc[1] + a_0;
+            row_acc[1] = a_p;
+            if (store_rho) ro_y[zt * psy + ((row_lo ? btym : btyp) * 2 + (row_lo ? 1 : 0)) * nx + x] = out;
+            // corners: only c_z = 0 directions reach a diagonal tile, so the target plane is this plane
+            if (store_h && (lane_lo || lane_hi)) {
+                T* cxy = ro_xy + zl * psxy;
+                if (lane_hi && row_hi) cxy[(btyp * ntx + btxp) * 4 + 0] = f[7];     // +x+y
+                if (lane_lo && row_lo) cxy[(btym * ntx + btxm) * 4 + 3] = f[8];     // -x-y
+                if (lane_hi && row_lo) cxy[(btym * ntx + btxp) * 4 + 2] = f[9];     // +x-y
+                if (lane_lo && row_hi) cxy[(btyp * ntx + btxm) * 4 + 1] = f[10];    // -x+y
+            }
+        }
+
+        mbar_wait(pub, it & 1);
 
         // ---- y stage and z pipeline of the gather; exports across the tile's x edges ----
-#pragma unroll
-        for (int k = 0; k < 2; ++k) {
+        {
             T a[3];
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                a[d] = u0[k][d];
-                if (ty > 0) a[d] += SU[(k * 6 + d) * SUP + own_s - RW];            // Up[dz](y-1)
-                if (ty < TY - 1) a[d] += SU[(k * 6 + 3 + d) * SUP + own_s + RW];   // Um[dz](y+1)
+                a[d] = u0[d];
+                if (!row_lo) a[d] += SU[d * SUP + own_s - RW];             // Up[dz](y-1)
+                if (!row_hi) a[d] += SU[(3 + d) * SUP + own_s + RW];       // Um[dz](y+1)
             }
-            const T out = own_acc[k][0] + a[0];
-            own_acc[k][0] = own_acc[k][1] + a[1];
-            own_acc[k][1] = a[2];
-            if (store_rho) ro.in[k * ro.s_in + (long long)zt * pl + own_xy] = out;
-            if (tx == 0 || tx == TX - 1) {
-                const bool lo = tx == 0;
-                const int vc = lo ? own_s - 1 : own_s + 1;                 // the virtual column next to this lane
-                T a_0 = ee[k][1];
-                if (ty > 0) a_0 += SU[(k * 6 + 1) * SUP + vc - RW];
-                if (ty < TY - 1) a_0 += SU[(k * 6 + 4) * SUP + vc + RW];
-                const T hout = col_acc[k][0] + ee[k][0];
-                col_acc[k][0] = col_acc[k][1] + a_0;
-                col_acc[k][1] = ee[k][2];
-                if (store_rho) ro.x[k * ro.s_x + zt * psx + ((bty * ntx + (lo ? btxm : btxp)) * 2 + (lo ? 1 : 0)) * TY + ty] = hout;
+            const T out = own_acc[0] + a[0];
+            own_acc[0] = own_acc[1] + a[1];
+            own_acc[1] = a[2];
+            if (store_rho) ro_in[(long long)zt * pl] = out;
+            if (lane_lo || lane_hi) {
+                const int vc = lane_lo ? own_s - 1 : own_s + 1;            // the virtual column next to this lane
+                T a_0 = ee[1];
+                if (!row_lo) a_0 += SU[1 * SUP + vc - RW];
+                if (!row_hi) a_0 += SU[4 * SUP + vc + RW];
+                const T hout = col_acc[0] + ee[0];
+                col_acc[0] = col_acc[1] + a_0;
+                col_acc[1] = ee[2];
+                if (store_rho) ro_x[zt * psx + ((bty * ntx + (lane_lo ? btxm : btxp)) * 2 + (lane_lo ? 1 : 0)) * TY + ty] = hout;
             }
         }
         if (it <= niter - 3) ring_load(z0 + 2 + it);                       // plane z+3
