@@ -49,7 +49,7 @@ struct lb_ctx {
     int kernel;        // resolved LB_KERNEL_*
     int kernel_req;
     int zc;            // planes per CTA of the one-pass kernel
-    CUtensorMap tmap[2][2];   // [buffer][narrow box 32 x TY, wide box (32 + 16 B) x TY] over [k*19+i][z][y][x]
+    CUtensorMap tmap[2][3];   // [buffer][narrow box 32 x TY, wide box (32 + 16 B) x TY, wrapped-column box 16 B x TY] over [k*19+i][z][y][x]
     bool have_tmap;
     double* stage;     // device staging, STAGE_NODES * 5 doubles
     double* diag_part; // [DIAG_BLOCKS][5]
@@ -533,8 +533,9 @@ bool make_tmaps(lb_ctx* c) {
     const cuuint32_t estr[4] = {1, 1, 1, 1};
     const CUtensorMapDataType dt = c->dtype == LB_F64 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     for (int b = 0; b < 2; ++b)
-        for (int w = 0; w < 2; ++w) {
-            const cuuint32_t box[4] = {cuuint32_t(OP_TX + (w ? 16 / int(es) : 0)), cuuint32_t(OP_TY), 1, 1};
+        for (int w = 0; w < 3; ++w) {
+            const cuuint32_t pad = cuuint32_t(16 / int(es));
+            const cuuint32_t box[4] = {w == 0 ? cuuint32_t(OP_TX) : (w == 1 ? OP_TX + pad : pad), cuuint32_t(OP_TY), 1, 1};
             if (enc(&c->tmap[b][w], dt, 4, c->f[b], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
                 return false;
@@ -553,7 +554,7 @@ int launch_tma(lb_ctx* c) {
     }
     const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc - 1) / c->zc);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], static_cast<const T*>(c->f[c->cur]),
+    kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                         static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                         rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
                                                         c->zc, om_r, om_b, G);

@@ -3,26 +3,29 @@
 // Same algorithm and same state convention as lb_onepass.cuh (h-state, pull streaming, density carried
 // from step to step through the four single-writer arrays rho_in / rho_x / rho_y / rho_xy), but the
 // 38 population planes of a tile are brought into shared memory by the TMA unit instead of by 38
-// per-thread loads:
+// per-thread loads, and one thread handles one (node, component) instead of one node:
 //   * one producer warp per CTA issues, per z plane, 38 `cp.async.bulk.tensor.4d` box loads (one per
-//     population plane, box = tile shifted by -c_i in y and z) that complete on an mbarrier; the TX*TY
-//     consumer threads then read their 38 values with immediate-offset LDS: no per-thread address
+//     population plane, box = tile shifted by -c_i in y and z) that complete on an mbarrier; the
+//     consumer threads then read their 19 values with LDS at fixed offsets: no per-thread address
 //     arithmetic, no registers in flight, and the prefetch distance is a whole plane whatever the
 //     occupancy is;
 //   * measured on B200: a TMA box whose innermost start is not 16-byte aligned
 //     raises an illegal-instruction fault, so the x shift cannot be given to the TMA.  Directions with
 //     c_x != 0 are loaded as an ALIGNED box that is PADX = 16/sizeof(T) elements wider, and the consumer
 //     applies the shift in its LDS address (free);
-//   * the TMA zero-fills out-of-range box parts and does not wrap: in tiles that touch the
-//     box boundary in x or y the producer warp patches the wrapped column / row from global memory after
-//     the box has landed and releases the consumers through a second mbarrier.  z wraps in the
-//     coordinate;
+//   * the TMA zero-fills out-of-range box parts and does not wrap.  x: tiles at the box
+//     boundary load, per direction with c_x != 0, one more box (PADX x TY) holding the wrapped column,
+//     and the lane next to the edge reads that box instead (a different base offset, same instruction).
+//     y: the one warp whose row lies beyond the edge re-loads its 5 affected populations with plain loads.
+//     z wraps in the box coordinate;
 //   * consumers copy the stage into registers and release it at once, so one stage buffers a whole
 //     plane of prefetch; post-collision values are stored straight from registers (aligned, coalesced);
-//   * one named barrier per plane (the y stage of the density gather, double-buffered), none for the
-//     stage hand-off (mbarriers).
-//
-// One CTA = TX*TY consumer threads (one node each, one warp per tile row) + 1 producer warp.
+//   * the two threads of a node exchange rho^k, j^k through shared memory (common velocity, S4) with a
+//     64-thread named barrier per tile row; the y stage of the density gather is double-buffered behind
+//     one split-phase mbarrier per plane (arrive, independent stores, wait); the stage hand-off is
+//     mbarriers only;
+//   * the producer warp group gives most of its registers to the consumers (setmaxnreg): 16 consumer
+//     warps at 112 registers.
 #pragma once
 #include <cuda.h>
 
@@ -65,7 +68,9 @@ struct TmaLayout {
     static constexpr int RW = TX + 2, RH = TY + 2, RS = RW * RH;       // density ring plane: tile + one-node frame
     static constexpr int SUP = TY * RW;                                // one y-stage plane: tile rows with an x frame
     __host__ __device__ static constexpr int align128(int elems) { return (elems * int(sizeof(T)) + 127) / 128 * 128 / int(sizeof(T)); }
-    static constexpr int NA = align128(NT), WA = align128(W * TY);     // slot sizes: narrow (c_x = 0) and wide boxes, 128-byte multiples
+    static constexpr int XC = W * TY;                                  // offset of the wrapped-column box inside a wide slot
+    static constexpr int NA = align128(NT), WA = align128((W + PADX) * TY);   // slot sizes: narrow (c_x = 0) and wide (+ wrapped column), 128-byte multiples
+    static_assert((XC * sizeof(T)) % 128 == 0, "the wrapped-column box must start 128-byte aligned");
     // number of wide slots before direction i (the directions with c_x != 0 are 1, 2, 7..14)
     __host__ __device__ static constexpr int wide_before(int i) { return (i > 1) + (i > 2) + (i > 7 ? (i - 7 < 8 ? i - 7 : 8) : 0); }
     __host__ __device__ static constexpr int slot_off(int q) {         // element offset of population plane q = k*19 + i
@@ -74,6 +79,7 @@ struct TmaLayout {
     static constexpr int STAGE = 0;
     static constexpr int STAGE_ELEMS = slot_off(NPOP);
     static constexpr unsigned STAGE_TX_BYTES = unsigned(2 * (9 * NT + 10 * W * TY) * sizeof(T));   // bytes the 38 boxes deliver
+    static constexpr unsigned XCOL_TX_BYTES = unsigned(2 * 5 * PADX * TY * sizeof(T));             // ... plus the 10 wrapped-column boxes of one x side
     static constexpr int RING = STAGE + STAGE_ELEMS;                   // [4][2][RS]      rho(t), planes z-1..z+2
     static constexpr int SU = RING + 8 * RS;                           // [2][2][6][SUP]  double-buffered Up[dz], Um[dz] per component
     static constexpr int XM = SU + 24 * SUP;                           // [2][NT][4]      rho^k, j^k of every node, exchanged between the two components' threads
@@ -81,10 +87,6 @@ struct TmaLayout {
     static constexpr int END = RP + 16 * NT;
     static constexpr size_t BAR_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
     static constexpr size_t BYTES = BAR_BYTE_OFF + 8 * sizeof(unsigned long long);
-    // where consumer (tx, ty) finds f_i = h_i(x - c_i) inside slot i
-    __host__ __device__ static constexpr int read_off(int i, int tx, int ty) {
-        return dir_cx(i) == 0 ? ty * TX + tx : ty * W + tx + (dir_cx(i) > 0 ? PADX - 1 : 1);
-    }
 };
 
 
@@ -95,7 +97,7 @@ struct TmaLayout {
 template <typename T, bool HAS_SOLID, int TY>
 __global__ void __launch_bounds__(2 * 32 * TY + 128, 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
-           const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
+           const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
            T om_r, T om_b, T G) {
     using L = TmaLayout<T, TY>;
@@ -114,7 +116,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     T* xm = sm + L::XM;
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma + L::BAR_BYTE_OFF);
     unsigned long long* full = bars;          // the 38 boxes of the next plane have landed (tx bytes)
-    unsigned long long* patch = bars + 1;     // ... and the producer has patched the wrapped column / row (boundary tiles)
     unsigned long long* done = bars + 2;      // every consumer warp has copied its part of the stage into registers
     unsigned long long* pub = bars + 3;       // every consumer warp has published its y-stage inputs of this plane
 
@@ -126,12 +127,12 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const int z1 = min(z0 + zc, nz);
     const int niter = z1 - z0 + 2;            // planes z0-1 .. z1; the first and the last are re-collided only
     const long long pl = (long long)nx * ny;
-    const bool wrap_tile = btx == 0 || btx == ntx - 1 || bty == 0 || bty == nty - 1;
+    const bool wrap_xlo = btx == 0, wrap_xhi = btx == ntx - 1;             // the TMA zero-fills outside the box: x wraps with an
+                                                                           // extra box per direction, y with consumer loads
     auto wrapz = [&](int p) { p %= nz; return p < 0 ? p + nz : p; };
 
     if (t == 0) {
         mbar_init(full, 1);
-        mbar_init(patch, 1);
         mbar_init(done, 2 * TY);
         mbar_init(pub, 2 * TY);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -148,49 +149,22 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
             if (lane == 0) {
                 if (j > 0) mbar_wait(done, (j - 1) & 1);
-                mbar_expect_tx(full, L::STAGE_TX_BYTES);
+                mbar_expect_tx(full, L::STAGE_TX_BYTES + (wrap_xlo ? L::XCOL_TX_BYTES : 0u) + (wrap_xhi ? L::XCOL_TX_BYTES : 0u));
 #pragma unroll
                 for (int q = 0; q < NPOP; ++q) {
                     const int i = q % Q;
                     const int zq = zw[1 - dir_cz(i)];                       // f_i(x) = h_i(x - c_i)
-                    if (dir_cx(i) == 0) tma_load_4d(stage + L::slot_off(q), &tm_n, full, x0, y0 - dir_cy(i), zq, q);
-                    else tma_load_4d(stage + L::slot_off(q), &tm_w, full, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zq, q);
+                    T* slot = stage + L::slot_off(q);
+                    if (dir_cx(i) == 0) tma_load_4d(slot, &tm_n, full, x0, y0 - dir_cy(i), zq, q);
+                    else {
+                        tma_load_4d(slot, &tm_w, full, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zq, q);
+                        // the column beyond the box edge: columns nx-PADX..nx-1 for c_x > 0, 0..PADX-1 for c_x < 0
+                        if (dir_cx(i) > 0 && wrap_xlo) tma_load_4d(slot + L::XC, &tm_c, full, nx - PADX, y0 - dir_cy(i), zq, q);
+                        if (dir_cx(i) < 0 && wrap_xhi) tma_load_4d(slot + L::XC, &tm_c, full, 0, y0 - dir_cy(i), zq, q);
+                    }
                 }
             }
             __syncwarp();
-            if (wrap_tile) {                                                // the TMA zero-filled what lies outside the box
-                mbar_wait(full, j & 1);
-#pragma unroll
-                for (int q = 0; q < NPOP; ++q) {
-                    const int i = q % Q;
-                    const int cx = dir_cx(i), cy = dir_cy(i);
-                    if (cx == 0 && cy == 0) continue;
-                    const T* src = h + (long long)q * NP + (long long)zw[1 - dir_cz(i)] * pl;
-                    T* slot = stage + L::slot_off(q);
-                    const int rowlen = cx == 0 ? TX : W;
-                    const int ox = cx > 0 ? x0 - PADX : x0;                 // global x of slot column 0
-                    if (cx != 0 && ((cx > 0 && btx == 0) || (cx < 0 && btx == ntx - 1))) {
-                        const int col = cx > 0 ? PADX - 1 : TX;             // the one column a consumer reads outside [0, nx)
-                        const int gx = cx > 0 ? nx - 1 : 0;
-                        if (lane < TY) {
-                            int gy = y0 - cy + lane;
-                            gy = gy < 0 ? gy + ny : (gy >= ny ? gy - ny : gy);
-                            slot[lane * rowlen + col] = src[(long long)gy * nx + gx];
-                        }
-                    }
-                    if (cy != 0 && ((cy > 0 && bty == 0) || (cy < 0 && bty == nty - 1))) {
-                        const int row = cy > 0 ? 0 : TY - 1;
-                        const int gy = cy > 0 ? ny - 1 : 0;
-                        for (int c = lane; c < rowlen; c += 32) {
-                            int gx = ox + c;
-                            gx = gx < 0 ? gx + nx : (gx >= nx ? gx - nx : gx);
-                            slot[row * rowlen + c] = src[(long long)gy * nx + gx];
-                        }
-                    }
-                }
-                __syncwarp();
-                if (lane == 0) mbar_arrive(patch);
-            }
         }
         return;
     }
@@ -219,6 +193,12 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     T* ro_y = ro.y + k * ro.s_y;
     T* ro_xy = ro.xy + k * ro.s_xy;
     const bool lane_lo = tx == 0, lane_hi = tx == TX - 1, row_lo = ty == 0, row_hi = ty == TY - 1;
+    // where this thread finds f_i = h_i(x - c_i) inside slot i, by c_x: the x shift is applied here; the lane next to the
+    // box edge reads the wrapped-column box instead
+    const int rd0 = ty * TX + tx;
+    const int rdp = (wrap_xlo && lane_lo) ? L::XC + ty * PADX + PADX - 1 : ty * W + tx + PADX - 1;
+    const int rdm = (wrap_xhi && lane_hi) ? L::XC + ty * PADX : ty * W + tx + 1;
+    const bool wrap_ylo = bty == 0 && row_lo, wrap_yhi = bty == nty - 1 && row_hi;   // warp-uniform
 
     // ---- density ring: every consumer owns ring positions tl and tl + NT of its component and assembles them
     //      from the four single-writer arrays in the fixed order ((in + x) + y) + xy ----
@@ -296,10 +276,20 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
 
         // ---- pull: the stage holds h_i(x - c_i) for the whole tile (Eq. 5, periodic) ----
         mbar_wait(full, it & 1);
-        if (wrap_tile) mbar_wait(patch, it & 1);
         T f[Q];
 #pragma unroll
-        for (int i = 0; i < Q; ++i) f[i] = stage_k[L::slot_off(i) + L::read_off(i, tx, ty)];
+        for (int i = 0; i < Q; ++i) f[i] = stage_k[L::slot_off(i) + (dir_cx(i) == 0 ? rd0 : (dir_cx(i) > 0 ? rdp : rdm))];
+        if (wrap_ylo || wrap_yhi) {                     // the row beyond the box edge in y (one warp of a boundary tile): plain loads
+            const int gy = wrap_ylo ? ny - 1 : 0;
+            const int xs[3] = {x == 0 ? nx - 1 : x - 1, x, x == nx - 1 ? 0 : x + 1};
+            const long long zs[3] = {(long long)zt * pl, zoff, (long long)(zl + 1 == nz ? 0 : zl + 1) * pl};
+#pragma unroll
+            for (int i = 1; i < Q; ++i)
+                if (dir_cy(i) != 0) {
+                    const T v = __ldg(hk + (long long)i * NP + zs[1 - dir_cz(i)] + (long long)gy * nx + xs[1 - dir_cx(i)]);
+                    if ((dir_cy(i) > 0 && wrap_ylo) || (dir_cy(i) < 0 && wrap_yhi)) f[i] = v;
+                }
+        }
         if (HAS_SOLID && (lk & 0x7FFFEu)) {             // halfway bounce-back (Eq. 23-24, u_b = 0): f_i(x) = h_opp(i)(x) when x - c_i is solid
 #pragma unroll
             for (int i = 1; i < Q; ++i)
