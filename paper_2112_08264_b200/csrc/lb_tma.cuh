@@ -56,6 +56,11 @@ __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, vo
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
                  ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+// the same box, into L2 only
+__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* tm, int c0, int c1, int c2, int c3) {
+    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
+                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 template <int ID, int COUNT>
 __device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(COUNT) : "memory"); }
 
@@ -161,6 +166,15 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                         // the column beyond the box edge: columns nx-PADX..nx-1 for c_x > 0, 0..PADX-1 for c_x < 0
                         if (dir_cx(i) > 0 && wrap_xlo) tma_load_4d(slot + L::XC, &tm_c, full, nx - PADX, y0 - dir_cy(i), zq, q);
                         if (dir_cx(i) < 0 && wrap_xhi) tma_load_4d(slot + L::XC, &tm_c, full, 0, y0 - dir_cy(i), zq, q);
+                    }
+                }
+                if (j + 1 < niter) {                                        // the plane after that: DRAM -> L2 now, so that its
+                    const int zn[3] = {zw[1], zw[2], wrapz(z + 2)};         // box loads (one stage, issued late) hit in L2
+#pragma unroll
+                    for (int q = 0; q < NPOP; ++q) {
+                        const int i = q % Q;
+                        if (dir_cx(i) == 0) tma_prefetch_4d(&tm_n, x0, y0 - dir_cy(i), zn[1 - dir_cz(i)], q);
+                        else tma_prefetch_4d(&tm_w, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zn[1 - dir_cz(i)], q);
                     }
                 }
             }
