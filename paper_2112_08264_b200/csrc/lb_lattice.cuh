@@ -67,6 +67,30 @@ __device__ __forceinline__ void collide19(T (&f)[Q], T rho, T omc, T ux, T uy, T
     }
 }
 
+// The same collision, handing every post-collision value to `emit(i, value)` as soon as it exists, so that the caller's
+// stores interleave with the arithmetic instead of queueing up behind it.
+template <typename T, typename Emit>
+__device__ __forceinline__ void collide19_emit(T (&f)[Q], T rho, T omc, T ux, T uy, T uz, T ex, T ey, T ez, Emit emit) {
+    const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    const T ae = T(1) - T(1.5) * (ex * ex + ey * ey + ez * ez);
+    f[0] = omc * f[0] + w_rest<T>() * rho * (ae - omc * a0);
+    emit(0, f[0]);
+#pragma unroll
+    for (int p = 0; p < 9; ++p) {
+        const T cu = T(pair_cx(p)) * ux + T(pair_cy(p)) * uy + T(pair_cz(p)) * uz;
+        const T ce = T(pair_cx(p)) * ex + T(pair_cy(p)) * ey + T(pair_cz(p)) * ez;
+        const T wr = w_pair<T>(p) * rho;
+        const T s0 = a0 + T(4.5) * cu * cu;
+        const T se = ae + T(4.5) * ce * ce;
+        const T sym = wr * (se - omc * s0);
+        const T asym = (T(3) * wr) * (ce - omc * cu);
+        f[2 * p + 1] = omc * f[2 * p + 1] + (sym + asym);
+        f[2 * p + 2] = omc * f[2 * p + 2] + (sym - asym);
+        emit(2 * p + 1, f[2 * p + 1]);
+        emit(2 * p + 2, f[2 * p + 2]);
+    }
+}
+
 // Eq. 10 for all 19 directions.
 template <typename T>
 __device__ __forceinline__ void equilibrium19(T (&f)[Q], T rho, T ux, T uy, T uz) {

@@ -86,14 +86,31 @@ struct TmaLayout {
     static constexpr unsigned STAGE_TX_BYTES = unsigned(2 * (9 * NT + 10 * W * TY) * sizeof(T));   // bytes the 38 boxes deliver
     static constexpr unsigned XCOL_TX_BYTES = unsigned(2 * 5 * PADX * TY * sizeof(T));             // ... plus the 10 wrapped-column boxes of one x side
     static constexpr int RING = STAGE + STAGE_ELEMS;                   // [4][2][RS]      rho(t), planes z-1..z+2
-    static constexpr int SU = RING + 8 * RS;                           // [2][2][6][SUP]  double-buffered Up[dz], Um[dz] per component
-    static constexpr int XM = SU + 24 * SUP;                           // [2][NT][4]      rho^k, j^k of every node, exchanged between the two components' threads
-    static constexpr int RP = XM + 8 * NT;                             // [8][2*NT]       thread-private landing slots of the ring pieces (cp.async)
-    static constexpr int END = RP + 16 * NT;
-    static constexpr size_t BAR_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
+    static constexpr int SU = RING + 8 * RS;                           // [2][2][2][SUP]  double-buffered z-summed Up, Um per component
+    static constexpr int XM = SU + 8 * SUP;                           // [2][NT][4]      rho^k, j^k of every node, exchanged between the two components' threads
+    // ring pieces: every ring position has an `in` piece; the positions in the 4 columns / 4 rows next to a tile edge
+    // also have an x / y piece, the 16 where they cross an xy piece
+    static constexpr int NEX = 4 * RH, NEY = 4 * RW, NEXY = 16;
+    static constexpr int RP_IN = XM + 8 * NT;                          // [2][RS]    landing slots of the pieces (cp.async), per component
+    static constexpr int RP_X = RP_IN + 2 * RS;                        // [2][NEX]
+    static constexpr int RP_Y = RP_X + 2 * NEX;                        // [2][NEY]
+    static constexpr int RP_XY = RP_Y + 2 * NEY;                       // [2][NEXY]
+    static constexpr int END = RP_XY + 2 * NEXY;
+    static constexpr size_t TAB_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
+    // int tables: T_IN[RS] offset of the in piece inside a plane; T_PK[RS] packed list indices (x | y << 8 | xy << 16, 255 = none);
+    // T_X[NEX], T_Y[NEY], T_XY[NEXY] offsets of the edge pieces inside their arrays' planes
+    static constexpr int T_IN = 0, T_PK = RS, T_X = 2 * RS, T_Y = T_X + NEX, T_XY = T_Y + NEY, T_END = T_XY + NEXY;
+    static constexpr size_t BAR_BYTE_OFF = (TAB_BYTE_OFF + size_t(T_END) * sizeof(int) + 15) / 16 * 16;
     static constexpr size_t BYTES = BAR_BYTE_OFF + 8 * sizeof(unsigned long long);
 };
 
+
+#ifdef LB_TMA_TRACE
+__device__ long long g_trace[64 * 16];
+#define TRACE(cond, it, slot) do { if ((cond) && blockIdx.x == 1 && blockIdx.y == 1 && blockIdx.z == 0 && (it) >= 0 && (it) < 64) g_trace[(it) * 16 + (slot)] = clock64(); } while (0)
+#else
+#define TRACE(cond, it, slot) do { } while (0)
+#endif
 
 // ---- the kernel ------------------------------------------------------------------------------------------
 // Threads: 2*NT consumers (component k = t / NT, node (tx, ty) = ((t % NT) % 32, (t % NT) / 32): one warp per
@@ -108,10 +125,11 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     using L = TmaLayout<T, TY>;
     constexpr int TX = L::TX, NT = L::NT, NC = 2 * NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     static_assert(RS <= 2 * NT, "ring fill: at most two positions per consumer thread");
+    static_assert(2 * L::NEX <= 96 && 2 * L::NEXY <= 96, "one ring thread per x / xy piece");
     static_assert(TY >= 2 && TY <= 8, "one named barrier per tile row (ids 1..TY)");
     // register hand-over between the warp groups: (2*NT + 128) threads start with 65536 / threads registers each
     constexpr int START_REGS = (65536 / (NC + 128)) / 8 * 8;
-    constexpr int PRODUCER_REGS = 32;
+    constexpr int PRODUCER_REGS = 64;
     constexpr int CONSUMER_REGS = (START_REGS + (START_REGS - PRODUCER_REGS) * 128 / NC) / 8 * 8;
     extern __shared__ __align__(1024) unsigned char smem_tma[];
     T* sm = reinterpret_cast<T*>(smem_tma);
@@ -123,6 +141,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     unsigned long long* full = bars;          // the 38 boxes of the next plane have landed (tx bytes)
     unsigned long long* done = bars + 2;      // every consumer warp has copied its part of the stage into registers
     unsigned long long* pub = bars + 3;       // every consumer warp has published its y-stage inputs of this plane
+    unsigned long long* rdy = bars + 4;       // the producer warp has assembled the density ring plane this iteration needs
+    int* tab = reinterpret_cast<int*>(smem_tma + L::TAB_BYTE_OFF);
 
     const int t = threadIdx.x;
     const int ntx = nx / TX, nty = ny / TY;
@@ -140,20 +160,123 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         mbar_init(full, 1);
         mbar_init(done, 2 * TY);
         mbar_init(pub, 2 * TY);
+        mbar_init(rdy, 3);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // ---- density ring bookkeeping: ring position pos (tile + one-node frame) of either component is the sum
+    //      ((in + x) + y) + xy of up to four single-writer pieces (lb_onepass.cuh); where they live, tabulated once ----
+    for (int pos = t; pos < RS; pos += blockDim.x) {
+        const int rx = pos % RW - 1, ry = pos / RW - 1;
+        const int txm = btx == 0 ? ntx - 1 : btx - 1, txp = btx == ntx - 1 ? 0 : btx + 1;
+        const int tym = bty == 0 ? nty - 1 : bty - 1, typ = bty == nty - 1 ? 0 : bty + 1;
+        const int otx = rx < 0 ? txm : (rx >= TX ? txp : btx), oty = ry < 0 ? tym : (ry >= TY ? typ : bty);
+        const int lx = rx < 0 ? TX - 1 : (rx >= TX ? 0 : rx), ly = ry < 0 ? TY - 1 : (ry >= TY ? 0 : ry);
+        const int c4 = rx == -1 ? 0 : (rx == 0 ? 1 : (rx == TX - 1 ? 2 : (rx == TX ? 3 : -1)));   // edge column / row of the tile grid
+        const int r4 = ry == -1 ? 0 : (ry == 0 ? 1 : (ry == TY - 1 ? 2 : (ry == TY ? 3 : -1)));
+        tab[L::T_IN + pos] = (oty * TY + ly) * nx + otx * TX + lx;
+        int pk = 0xFFFFFF;
+        if (c4 >= 0) {
+            const int m = c4 * L::RH + ry + 1;
+            tab[L::T_X + m] = ((oty * ntx + otx) * 2 + (lx != 0)) * TY + ly;
+            pk = (pk & ~0xFF) | m;
+        }
+        if (r4 >= 0) {
+            const int m = r4 * RW + rx + 1;
+            tab[L::T_Y + m] = (oty * 2 + (ly != 0)) * nx + otx * TX + lx;
+            pk = (pk & ~0xFF00) | (m << 8);
+        }
+        if (c4 >= 0 && r4 >= 0) {
+            const int m = r4 * 4 + c4;
+            tab[L::T_XY + m] = (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
+            pk = (pk & ~0xFF0000) | (m << 16);
+        }
+        tab[L::T_PK + pos] = pk;
     }
     __syncthreads();
 
     // =================================== producer warp ===================================
     if (t >= NC) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(PRODUCER_REGS));
-        if (t >= NC + 32) return;
+        if (t >= NC + 32) {
+            // ---- ring warps (3): assemble the density ring, one plane per iteration, two planes ahead of its use ----
+            const int r = t - NC - 32;
+            constexpr int NR = 96;
+            const long long psx_ = (long long)nty * ntx * 2 * TY, psy_ = (long long)nty * 2 * nx, psxy_ = (long long)nty * ntx * 4;
+            T* s_in = sm + L::RP_IN;
+            T* s_x = sm + L::RP_X;
+            T* s_y = sm + L::RP_Y;
+            T* s_xy = sm + L::RP_XY;
+            auto ring_sync = [&]() { asm volatile("bar.sync %0, %1;" ::"n"(TY + 2), "n"(NR) : "memory"); };
+            // ask for the pieces of ring plane rp (= box plane z0 - 2 + rp): asynchronous, no registers in flight
+            auto ring_fetch = [&](int rp) {
+                const long long zp = wrapz(z0 - 2 + rp);
+#pragma unroll
+                for (int kk = 0; kk < 2; ++kk) {
+                    const T* b_in = ri.in + kk * ri.s_in + zp * pl;
+                    for (int pos = r; pos < RS; pos += NR) cp_async<sizeof(T)>(s_in + kk * RS + pos, b_in + tab[L::T_IN + pos]);
+                    const T* b_y = ri.y + kk * ri.s_y + zp * psy_;
+                    for (int m = r; m < L::NEY; m += NR) cp_async<sizeof(T)>(s_y + kk * L::NEY + m, b_y + tab[L::T_Y + m]);
+                }
+                if (r < 2 * L::NEX) {
+                    const int kk = r >= L::NEX, m = r - kk * L::NEX;
+                    cp_async<sizeof(T)>(s_x + r, ri.x + kk * ri.s_x + zp * psx_ + tab[L::T_X + m]);
+                }
+                if (r >= NR - 2 * L::NEXY) {
+                    const int q = r - (NR - 2 * L::NEXY), kk = q >= L::NEXY, m = q - kk * L::NEXY;
+                    cp_async<sizeof(T)>(s_xy + q, ri.xy + kk * ri.s_xy + zp * psxy_ + tab[L::T_XY + m]);
+                }
+                cp_async_commit();
+            };
+            // ... and add them up in the fixed order ((in + x) + y) + xy once they have landed
+            auto ring_assemble = [&](int rp) {
+                cp_async_wait<0>();
+                TRACE(r == 0, rp - 2, 14);
+                ring_sync();                                               // every ring thread's pieces are in
+                TRACE(r == 0, rp - 2, 15);
+                T* dst = ring + (rp & 3) * 2 * RS;
+#pragma unroll
+                for (int kk = 0; kk < 2; ++kk)
+                    for (int pos = r; pos < RS; pos += NR) {
+                        T v = s_in[kk * RS + pos];
+                        const int pk = tab[L::T_PK + pos];
+                        if (pk != 0xFFFFFF) {
+                            const int ix = pk & 255, iy = (pk >> 8) & 255, ixy = (pk >> 16) & 255;
+                            if (ix != 255) v += s_x[kk * L::NEX + ix];
+                            if (iy != 255) v += s_y[kk * L::NEY + iy];
+                            if (ixy != 255) v += s_xy[kk * L::NEXY + ixy];
+                        }
+                        dst[kk * RS + pos] = v;
+                    }
+                TRACE(r == 0, rp - 2, 11);
+                ring_sync();                                               // the landing slots may be overwritten
+            };
+            for (int rp = 0; rp < 2; ++rp) {                                // iteration 0 needs ring planes 0, 1, 2
+                ring_fetch(rp);
+                ring_assemble(rp);
+            }
+            ring_fetch(2);
+            for (int j = 0; j < niter; ++j) {
+                // ring plane j+2 (the z+1 neighbour plane of iteration j): its slot held plane j-2, last read in iteration
+                // j-2, which every consumer warp had left when it arrived on done(j-1)
+                if (j > 0) mbar_wait(done, (j - 1) & 1);
+                TRACE(r == 0, j, 8);
+                ring_assemble(j + 2);
+                __syncwarp();
+                if ((r & 31) == 0) mbar_arrive(rdy);
+                TRACE(r == 0, j, 9);
+                if (j + 3 <= niter + 1) ring_fetch(j + 3);
+                TRACE(r == 0, j, 10);
+            }
+            return;
+        }
+        // ---- TMA warp ----
         const int lane = t - NC;
         for (int j = 0; j < niter; ++j) {
             const int z = z0 - 1 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
             if (lane == 0) {
                 if (j > 0) mbar_wait(done, (j - 1) & 1);
+                TRACE(true, j, 12);
                 mbar_expect_tx(full, L::STAGE_TX_BYTES + (wrap_xlo ? L::XCOL_TX_BYTES : 0u) + (wrap_xhi ? L::XCOL_TX_BYTES : 0u));
 #pragma unroll
                 for (int q = 0; q < NPOP; ++q) {
@@ -178,6 +301,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                     }
                 }
             }
+            TRACE(lane == 0, j, 13);
             __syncwarp();
         }
         return;
@@ -201,7 +325,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const T* hk = h + (long long)k * Q * NP;
     T* gk = g + (long long)k * Q * NP + own_xy;
     const T* ring_o = ring + (1 - k) * RS;                                 // the OTHER component's density (S2)
-    T* SUk = SUb + k * 6 * SUP;
+    T* SUk = SUb + k * 2 * SUP;
     T* ro_in = ro.in + k * ro.s_in + own_xy;
     T* ro_x = ro.x + k * ro.s_x;
     T* ro_y = ro.y + k * ro.s_y;
@@ -214,66 +338,11 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const int rdm = (wrap_xhi && lane_hi) ? L::XC + ty * PADX : ty * W + tx + 1;
     const bool wrap_ylo = bty == 0 && row_lo, wrap_yhi = bty == nty - 1 && row_hi;   // warp-uniform
 
-    // ---- density ring: every consumer owns ring positions tl and tl + NT of its component and assembles them
-    //      from the four single-writer arrays in the fixed order ((in + x) + y) + xy ----
-    int o_in[2], o_x[2], o_y[2], o_xy[2];
-#pragma unroll
-    for (int a = 0; a < 2; ++a) {
-        const int pos = tl + a * NT;
-        o_in[a] = o_x[a] = o_y[a] = o_xy[a] = -1;
-        if (pos < RS) {
-            const int rx = pos % RW - 1, ry = pos / RW - 1;
-            const int otx = rx < 0 ? btxm : (rx >= TX ? btxp : btx), oty = ry < 0 ? btym : (ry >= TY ? btyp : bty);
-            const int lx = rx < 0 ? TX - 1 : (rx >= TX ? 0 : rx), ly = ry < 0 ? TY - 1 : (ry >= TY ? 0 : ry);
-            const bool ex = lx == 0 || lx == TX - 1, ey = ly == 0 || ly == TY - 1;
-            o_in[a] = (oty * TY + ly) * nx + otx * TX + lx;
-            if (ex) o_x[a] = ((oty * ntx + otx) * 2 + (lx != 0)) * TY + ly;
-            if (ey) o_y[a] = (oty * 2 + (ly != 0)) * nx + otx * TX + lx;
-            if (ex && ey) o_xy[a] = (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
-        }
-    }
-    const T* ri_in = ri.in + k * ri.s_in;
-    const T* ri_x = ri.x + k * ri.s_x;
-    const T* ri_y = ri.y + k * ri.s_y;
-    const T* ri_xy = ri.xy + k * ri.s_xy;
-    T* rp = sm + L::RP + t;                                                // [position*4 + piece][2*NT]: this thread's landing slots
-    auto ring_load = [&](int p) {                                          // asynchronous: no registers in flight
-        const long long zp = wrapz(p);
-#pragma unroll
-        for (int a = 0; a < 2; ++a) {
-            if (o_in[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 0) * NC, ri_in + zp * pl + o_in[a]);
-            if (o_x[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 1) * NC, ri_x + zp * psx + o_x[a]);
-            if (o_y[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 2) * NC, ri_y + zp * psy + o_y[a]);
-            if (o_xy[a] >= 0) cp_async<sizeof(T)>(rp + (a * 4 + 3) * NC, ri_xy + zp * psxy + o_xy[a]);
-        }
-        cp_async_commit();
-    };
-    auto ring_store = [&](int slot) {                                      // the same thread reads what it asked for: no barrier
-        cp_async_wait<0>();
-#pragma unroll
-        for (int a = 0; a < 2; ++a) {
-            if (o_in[a] < 0) continue;
-            T v = rp[(a * 4 + 0) * NC];
-            if (o_x[a] >= 0) v += rp[(a * 4 + 1) * NC];
-            if (o_y[a] >= 0) v += rp[(a * 4 + 2) * NC];
-            if (o_xy[a] >= 0) v += rp[(a * 4 + 3) * NC];
-            ring[(slot * 2 + k) * RS + tl + a * NT] = v;
-        }
-    };
-#pragma unroll 1
-    for (int p = 0; p < 3; ++p) {                                          // planes z0-2, z0-1, z0 -> slots 0, 1, 2
-        ring_load(z0 - 2 + p);
-        ring_store(p);
-    }
-    ring_load(z0 + 1);                                                     // stored in iteration 0
-    named_barrier<TY + 1, NC>();
-
     // ---- per-thread state carried along z ----
-    T own_acc[2] = {zero, zero};     // z pipeline of this node's gathered density: [0] = A_+1(z-2) + A_0(z-1), [1] = A_+1(z-1)
-    T row_acc[2] = {zero, zero};     // the same for the export across the tile's y edge (warps ty = 0 and TY-1)
-    T col_acc[2] = {zero, zero};     // ... across the tile's x edge (lanes tx = 0 and TX-1)
-    auto from_left = [&](T v) { const T r = __shfl_up_sync(0xffffffffu, v, 1); return lane_lo ? zero : r; };
-    auto from_right = [&](T v) { const T r = __shfl_down_sync(0xffffffffu, v, 1); return lane_hi ? zero : r; };
+    // z pipelines of the density gather, one per y class of the row sums (U0: c_y = 0, Up: c_y = +1, Um: c_y = -1):
+    // [0] = V_+1(z-2) + V_0(z-1), [1] = V_+1(z-1); adding V_-1(z) completes plane z-1
+    T acc0[2] = {zero, zero}, accp[2] = {zero, zero}, accm[2] = {zero, zero};
+    T col_acc[2] = {zero, zero};     // the same for the export across the tile's x edge (lanes tx = 0 and TX-1)
 
     int zl = wrapz(z0 - 1), zt = wrapz(z0 - 2);         // this plane / the plane the gathered density belongs to
     unsigned lk = 0;
@@ -286,10 +355,15 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         const bool store_rho = it >= 2;                 // target plane z-1 lies in [z0, z1)
         const int s0 = (it + 1) & 3;                    // ring slot of plane z
         const bool fluid = !HAS_SOLID || !(lk & OP_SOLID_BIT);   // nothing happens inside a particle
-        T* SU = SUk + (it & 1) * 12 * SUP;
+        T* SU = SUk + (it & 1) * 4 * SUP;
 
         // ---- pull: the stage holds h_i(x - c_i) for the whole tile (Eq. 5, periodic) ----
+        TRACE(t == 0, it, 0);
         mbar_wait(full, it & 1);
+        TRACE(t == 0, it, 1);
+        mbar_wait(rdy, it & 1);                         // density ring planes z-1, z, z+1 are in place (before `done`: the producer
+                                                        // must not get two phases ahead of any waiter)
+        TRACE(t == 0, it, 2);
         T f[Q];
 #pragma unroll
         for (int i = 0; i < Q; ++i) f[i] = stage_k[L::slot_off(i) + (dir_cx(i) == 0 ? rd0 : (dir_cx(i) > 0 ? rdp : rdm))];
@@ -310,6 +384,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                 if (lk >> dir_opp(i) & 1u) f[i] = __ldg(hk + (long long)dir_opp(i) * NP + zoff + own_xy);
         }
         __syncwarp();
+        TRACE(t == 0, it, 3);
         if (lane_lo) mbar_arrive(done);                 // the producer may refill the stage with the next plane
 
         // ---- moments of this component (Eq. 6-7), exchanged with the other component's thread of the same node ----
@@ -354,74 +429,72 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             }
             ex = ux - G * gx; ey = uy - G * gy; ez = uz - G * gz;
             // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) ----
-            collide19<T>(f, rho, omc, ux, uy, uz, ex, ey, ez);
+            //      each value is stored (aligned, coalesced) as soon as it exists
+            T* o = gk + zoff;
+            collide19_emit<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, [&](int i, T v) { if (store_h) o[(long long)i * NP] = v; });
         }
 
-        // ---- density gather, x stage (warp shuffles) and publication of the y-stage inputs ----
-        T u0[3] = {zero, f[0], zero};                    // U0[dz] row sums
+        // ---- density gather rho(y, t+1) = sum_i h_i(y - c_i): x by warp shuffles, z by register pipelines, y through
+        //      shared memory (two values per node) ----
+        T u0[3] = {zero, f[0], zero};                    // row sums by c_z, c_y = 0
         T ee[3] = {zero, zero, zero};                    // on lanes tx = 0 / TX-1: what leaves the tile in x with c_y = 0
-        T up[3] = {zero, zero, zero}, um[3] = {zero, zero, zero};
-        {
-            T* sup0 = SU + 1 * SUP;                      // Up[dz = 0]
-            T* sum0 = SU + 4 * SUP;                      // Um[dz = 0]
+        T up[3] = {zero, zero, zero}, um[3] = {zero, zero, zero};   // c_y = +1 / -1
+        T* SUup = SU;                                    // interior: Up summed over z (plane z-1); x frame: Up[c_z = 0] of the virtual column, plane z
+        T* SUum = SU + SUP;
 #pragma unroll
-            for (int p = 0; p < 9; ++p) {
-                const T h1 = f[2 * p + 1], h2 = f[2 * p + 2];
-                T l = zero, r = zero;
-                if (p == 0 || (p >= 3 && p <= 6)) { l = from_left(h1); r = from_right(h2); }
-                if (p == 0) {                                              // +x / -x
-                    u0[1] += l; u0[1] += r;
-                    ee[1] = lane_hi ? h1 : h2;
-                } else if (p == 1) { up[1] = h1; um[1] = h2; }              // +y / -y
-                else if (p == 2) { u0[2] = h1; u0[0] = h2; }                // +z / -z
-                else if (p == 3) {                                         // +x+y / -x-y
-                    up[1] += l; um[1] += r;
-                    if (lane_hi) sup0[own_s + 1] = h1;
-                    if (lane_lo) sum0[own_s - 1] = h2;
-                } else if (p == 4) {                                       // +x-y / -x+y
-                    um[1] += l; up[1] += r;
-                    if (lane_hi) sum0[own_s + 1] = h1;
-                    if (lane_lo) sup0[own_s - 1] = h2;
-                } else if (p == 5) {                                       // +x+z / -x-z
-                    u0[2] += l; u0[0] += r;
-                    if (lane_hi) ee[2] = h1;
-                    if (lane_lo) ee[0] = h2;
-                } else if (p == 6) {                                       // +x-z / -x+z
-                    u0[0] += l; u0[2] += r;
-                    if (lane_hi) ee[0] = h1;
-                    if (lane_lo) ee[2] = h2;
-                } else if (p == 7) { up[2] = h1; um[0] = h2; }              // +y+z / -y-z
-                else { up[0] = h1; um[2] = h2; }                           // +y-z / -y+z
-            }
-            if (HAS_SOLID && fluid && (lk & 0x7FFFEu)) {                   // bounced-back arrivals of the next step come from this node
-                T bs = zero;
-#pragma unroll
-                for (int i = 1; i < Q; ++i)
-                    if (lk >> i & 1u) bs += f[i];
-                u0[1] += bs;
-            }
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                SU[d * SUP + own_s] = up[d];
-                SU[(3 + d) * SUP + own_s] = um[d];
-            }
+        for (int p = 0; p < 9; ++p) {
+            const T h1 = f[2 * p + 1], h2 = f[2 * p + 2];
+            T l = zero, r = zero;
+            if (p == 0 || (p >= 3 && p <= 6)) { l = __shfl_up_sync(0xffffffffu, h1, 1); r = __shfl_down_sync(0xffffffffu, h2, 1); }
+            if (p == 0) {                                                  // +x / -x
+                if (!lane_lo) u0[1] += l;
+                if (!lane_hi) u0[1] += r;
+                ee[1] = lane_hi ? h1 : h2;
+            } else if (p == 1) { up[1] = h1; um[1] = h2; }                  // +y / -y
+            else if (p == 2) { u0[2] = h1; u0[0] = h2; }                    // +z / -z
+            else if (p == 3) {                                             // +x+y / -x-y
+                if (!lane_lo) up[1] += l;
+                if (!lane_hi) um[1] += r;
+                if (lane_hi) SUup[own_s + 1] = h1;
+                if (lane_lo) SUum[own_s - 1] = h2;
+            } else if (p == 4) {                                           // +x-y / -x+y
+                if (!lane_lo) um[1] += l;
+                if (!lane_hi) up[1] += r;
+                if (lane_hi) SUum[own_s + 1] = h1;
+                if (lane_lo) SUup[own_s - 1] = h2;
+            } else if (p == 5) {                                           // +x+z / -x-z
+                if (!lane_lo) u0[2] += l;
+                if (!lane_hi) u0[0] += r;
+                if (lane_hi) ee[2] = h1;
+                if (lane_lo) ee[0] = h2;
+            } else if (p == 6) {                                           // +x-z / -x+z
+                if (!lane_lo) u0[0] += l;
+                if (!lane_hi) u0[2] += r;
+                if (lane_hi) ee[0] = h1;
+                if (lane_lo) ee[2] = h2;
+            } else if (p == 7) { up[2] = h1; um[0] = h2; }                  // +y+z / -y-z
+            else { up[0] = h1; um[2] = h2; }                               // +y-z / -y+z
         }
-        if (it <= niter - 2) ring_store((it + 3) & 3);                     // rho(t) of plane z+2, loaded one iteration ago
+        if (HAS_SOLID && fluid && (lk & 0x7FFFEu)) {                       // bounced-back arrivals of the next step come from this node
+            T bs = zero;
+#pragma unroll
+            for (int i = 1; i < Q; ++i)
+                if (lk >> i & 1u) bs += f[i];
+            u0[1] += bs;
+        }
+        const T p0 = acc0[0] + u0[0], pp = accp[0] + up[0], pm = accm[0] + um[0];   // complete for plane z-1
+        acc0[0] = acc0[1] + u0[1]; acc0[1] = u0[2];
+        accp[0] = accp[1] + up[1]; accp[1] = up[2];
+        accm[0] = accm[1] + um[1]; accm[1] = um[2];
+        SUup[own_s] = pp;
+        SUum[own_s] = pm;
         __syncwarp();
         if (lane_lo) mbar_arrive(pub);
+        TRACE(t == 0, it, 4);
 
-        // ---- global stores that need nothing from the other warps: h, the y-edge and corner exports ----
-        if (fluid && store_h) {
-            T* o = gk + zoff;
-#pragma unroll
-            for (int i = 0; i < Q; ++i) o[(long long)i * NP] = f[i];
-        }
+        // ---- global stores that need nothing from the other warps: the y-edge and corner exports ----
         if (row_lo || row_hi) {                                            // the row beyond the tile edge receives exactly Um (Up)
-            const T a_m = row_lo ? um[0] : up[0], a_0 = row_lo ? um[1] : up[1], a_p = row_lo ? um[2] : up[2];
-            const T out = row_acc[0] + a_m;
-            row_acc[0] = row_acc[1] + a_0;
-            row_acc[1] = a_p;
-            if (store_rho) ro_y[zt * psy + ((row_lo ? btym : btyp) * 2 + (row_lo ? 1 : 0)) * nx + x] = out;
+            if (store_rho) ro_y[zt * psy + ((row_lo ? btym : btyp) * 2 + (row_lo ? 1 : 0)) * nx + x] = row_lo ? pm : pp;
             // corners: only c_z = 0 directions reach a diagonal tile, so the target plane is this plane
             if (store_h && (lane_lo || lane_hi)) {
                 T* cxy = ro_xy + zl * psxy;
@@ -432,33 +505,27 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             }
         }
 
+        TRACE(t == 0, it, 5);
         mbar_wait(pub, it & 1);
+        TRACE(t == 0, it, 6);
 
-        // ---- y stage and z pipeline of the gather; exports across the tile's x edges ----
+        // ---- y stage of the gather; exports across the tile's x edges ----
         {
-            T a[3];
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                a[d] = u0[d];
-                if (!row_lo) a[d] += SU[d * SUP + own_s - RW];             // Up[dz](y-1)
-                if (!row_hi) a[d] += SU[(3 + d) * SUP + own_s + RW];       // Um[dz](y+1)
-            }
-            const T out = own_acc[0] + a[0];
-            own_acc[0] = own_acc[1] + a[1];
-            own_acc[1] = a[2];
+            T out = p0;
+            if (!row_lo) out += SUup[own_s - RW];                          // Up(y-1)
+            if (!row_hi) out += SUum[own_s + RW];                          // Um(y+1)
             if (store_rho) ro_in[(long long)zt * pl] = out;
             if (lane_lo || lane_hi) {
                 const int vc = lane_lo ? own_s - 1 : own_s + 1;            // the virtual column next to this lane
                 T a_0 = ee[1];
-                if (!row_lo) a_0 += SU[1 * SUP + vc - RW];
-                if (!row_hi) a_0 += SU[4 * SUP + vc + RW];
+                if (!row_lo) a_0 += SUup[vc - RW];
+                if (!row_hi) a_0 += SUum[vc + RW];
                 const T hout = col_acc[0] + ee[0];
                 col_acc[0] = col_acc[1] + a_0;
                 col_acc[1] = ee[2];
                 if (store_rho) ro_x[zt * psx + ((bty * ntx + (lane_lo ? btxm : btxp)) * 2 + (lane_lo ? 1 : 0)) * TY + ty] = hout;
             }
         }
-        if (it <= niter - 3) ring_load(z0 + 2 + it);                       // plane z+3
         zt = zl;
         zl = zl + 1 == nz ? 0 : zl + 1;
         if (HAS_SOLID && it + 1 < niter) lk = __ldg(links + (long long)zl * pl + own_xy);
