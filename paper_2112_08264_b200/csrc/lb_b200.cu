@@ -49,6 +49,7 @@ struct lb_ctx {
     int kernel;        // resolved LB_KERNEL_*
     int kernel_req;
     int zc;            // planes per CTA of the one-pass kernel
+    int zc_tma;        // ... of the TMA kernel (one CTA per SM)
     CUtensorMap tmap[2][3];   // [buffer][narrow box 32 x TY, wide box (32 + 16 B) x TY, wrapped-column box 16 B x TY] over [k*19+i][z][y][x]
     bool have_tmap;
     double* stage;     // device staging, STAGE_NODES * 5 doubles
@@ -552,12 +553,12 @@ int launch_tma(lb_ctx* c) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
         configured = true;
     }
-    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc - 1) / c->zc);
+    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
     kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                         static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                         rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
-                                                        c->zc, om_r, om_b, G);
+                                                        c->zc_tma, om_r, om_b, G);
     c->launches += 1;
     CU(cudaGetLastError());
     return LB_OK;
@@ -572,6 +573,25 @@ int step_tma(lb_ctx* c) {
     c->cur ^= 1;
     c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
     return LB_OK;
+}
+
+// planes per CTA of the TMA kernel: every chunk re-collides 2 extra planes (long chunks), but the grid should fill the
+// SMs (one CTA each) in whole waves, and more waves balance better.  Measured on B200: 256^3 -> 64, 512^3 -> 256.
+int tma_zc(const lb_ctx* c) {
+    if (const char* e = std::getenv("LB_ONEPASS_ZC")) { const int v = std::atoi(e); if (v >= 1) return v < c->nz ? v : c->nz; }
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const double tiles = double(c->nx / OP_TX) * (c->ny / OP_TY);
+    int best = c->nz;
+    double best_cost = 1e300;
+    for (int zc = 1; zc <= c->nz; ++zc) {
+        if (c->nz % zc != 0) continue;
+        const int chunks = c->nz / zc;
+        const double full = std::ceil(tiles * chunks / sms);          // waves of CTAs
+        const double cost = full * (zc + 4) * (1.0 + 0.25 / full);     // planes collided + prologue, per SM; tail imbalance
+        if (cost < best_cost) { best_cost = cost; best = zc; }
+    }
+    return best;
 }
 
 int resolve_kernel(lb_ctx* c, int kind) {
@@ -663,6 +683,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
     c->zc = onepass_zc(c);
+    c->zc_tma = tma_zc(c);
     return c;
 }
 

@@ -327,9 +327,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const T* ring_o = ring + (1 - k) * RS;                                 // the OTHER component's density (S2)
     T* SUk = SUb + k * 2 * SUP;
     T* ro_in = ro.in + k * ro.s_in + own_xy;
-    T* ro_x = ro.x + k * ro.s_x;
-    T* ro_y = ro.y + k * ro.s_y;
-    T* ro_xy = ro.xy + k * ro.s_xy;
     const bool lane_lo = tx == 0, lane_hi = tx == TX - 1, row_lo = ty == 0, row_hi = ty == TY - 1;
     // where this thread finds f_i = h_i(x - c_i) inside slot i, by c_x: the x shift is applied here; the lane next to the
     // box edge reads the wrapped-column box instead
@@ -430,8 +427,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             ex = ux - G * gx; ey = uy - G * gy; ez = uz - G * gz;
             // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) ----
             //      each value is stored (aligned, coalesced) as soon as it exists
-            T* o = gk + zoff;
-            collide19_emit<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, [&](int i, T v) { if (store_h) o[(long long)i * NP] = v; });
+            T* o = gk + zoff;                                               // values arrive in direction order: a running pointer
+            collide19_emit<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, [&](int, T v) { if (store_h) *o = v; o += NP; });
         }
 
         // ---- density gather rho(y, t+1) = sum_i h_i(y - c_i): x by warp shuffles, z by register pipelines, y through
@@ -494,10 +491,10 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
 
         // ---- global stores that need nothing from the other warps: the y-edge and corner exports ----
         if (row_lo || row_hi) {                                            // the row beyond the tile edge receives exactly Um (Up)
-            if (store_rho) ro_y[zt * psy + ((row_lo ? btym : btyp) * 2 + (row_lo ? 1 : 0)) * nx + x] = row_lo ? pm : pp;
+            if (store_rho) (ro.y + k * ro.s_y)[zt * psy + ((row_lo ? btym : btyp) * 2 + (row_lo ? 1 : 0)) * nx + x] = row_lo ? pm : pp;
             // corners: only c_z = 0 directions reach a diagonal tile, so the target plane is this plane
             if (store_h && (lane_lo || lane_hi)) {
-                T* cxy = ro_xy + zl * psxy;
+                T* cxy = ro.xy + k * ro.s_xy + zl * psxy;
                 if (lane_hi && row_hi) cxy[(btyp * ntx + btxp) * 4 + 0] = f[7];     // +x+y
                 if (lane_lo && row_lo) cxy[(btym * ntx + btxm) * 4 + 3] = f[8];     // -x-y
                 if (lane_hi && row_lo) cxy[(btym * ntx + btxp) * 4 + 2] = f[9];     // +x-y
@@ -523,7 +520,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                 const T hout = col_acc[0] + ee[0];
                 col_acc[0] = col_acc[1] + a_0;
                 col_acc[1] = ee[2];
-                if (store_rho) ro_x[zt * psx + ((bty * ntx + (lane_lo ? btxm : btxp)) * 2 + (lane_lo ? 1 : 0)) * TY + ty] = hout;
+                if (store_rho) (ro.x + k * ro.s_x)[zt * psx + ((bty * ntx + (lane_lo ? btxm : btxp)) * 2 + (lane_lo ? 1 : 0)) * TY + ty] = hout;
             }
         }
         zt = zl;
