@@ -26,20 +26,26 @@ __host__ __device__ constexpr int dir_opp(int i) { return i == 0 ? 0 : ((i & 1) 
 template <typename T> __host__ __device__ constexpr T w_rest() { return T(1.0 / 3.0); }
 template <typename T> __host__ __device__ constexpr T w_pair(int p) { return p < 3 ? T(1.0 / 18.0) : T(1.0 / 36.0); }
 
+// c_p . v for the odd member of pair p, written without the multiplications by 0 and 1 that IEEE arithmetic does not
+// let the compiler drop (0 * x and 0 + x are not x for infinities / -0): p is a compile-time constant after unrolling.
+template <typename T>
+__device__ __forceinline__ T cdot(int p, T x, T y, T z) {
+    return p == 0 ? x : p == 1 ? y : p == 2 ? z : p == 3 ? x + y : p == 4 ? x - y : p == 5 ? x + z : p == 6 ? x - z : p == 7 ? y + z : y - z;
+}
+
 // rho = sum_i f_i and j = sum_i f_i c_i of one component (Eq. 6-7).
 template <typename T>
 __device__ __forceinline__ void moments19(const T (&f)[Q], T& rho, T& jx, T& jy, T& jz) {
-    T r = f[0], x = T(0), y = T(0), z = T(0);
+    T r = f[0], d[9];
 #pragma unroll
     for (int p = 0; p < 9; ++p) {
-        const T a = f[2 * p + 1], b = f[2 * p + 2];
-        r += a + b;
-        const T d = a - b;
-        if (pair_cx(p) > 0) x += d; else if (pair_cx(p) < 0) x -= d;
-        if (pair_cy(p) > 0) y += d; else if (pair_cy(p) < 0) y -= d;
-        if (pair_cz(p) > 0) z += d; else if (pair_cz(p) < 0) z -= d;
+        r += f[2 * p + 1] + f[2 * p + 2];
+        d[p] = f[2 * p + 1] - f[2 * p + 2];
     }
-    rho = r; jx = x; jy = y; jz = z;
+    rho = r;
+    jx = (((d[0] + d[3]) + d[4]) + d[5]) + d[6];       // pairs with c_x = +1
+    jy = (((d[1] + d[3]) - d[4]) + d[7]) + d[8];       // c_y = +1, +1, -1, +1, +1
+    jz = (((d[2] + d[5]) - d[6]) + d[7]) - d[8];       // c_z = +1, +1, -1, +1, -1
 }
 
 // BGK collision with exact-difference forcing (Eq. 1; Eq. 10, PAPER.md:338-342;
@@ -55,8 +61,8 @@ __device__ __forceinline__ void collide19(T (&f)[Q], T rho, T omc, T ux, T uy, T
     f[0] = omc * f[0] + w_rest<T>() * rho * (ae - omc * a0);
 #pragma unroll
     for (int p = 0; p < 9; ++p) {
-        const T cu = T(pair_cx(p)) * ux + T(pair_cy(p)) * uy + T(pair_cz(p)) * uz;
-        const T ce = T(pair_cx(p)) * ex + T(pair_cy(p)) * ey + T(pair_cz(p)) * ez;
+        const T cu = cdot<T>(p, ux, uy, uz);
+        const T ce = cdot<T>(p, ex, ey, ez);
         const T wr = w_pair<T>(p) * rho;
         const T s0 = a0 + T(4.5) * cu * cu;
         const T se = ae + T(4.5) * ce * ce;
@@ -77,8 +83,8 @@ __device__ __forceinline__ void collide19_emit(T (&f)[Q], T rho, T omc, T ux, T 
     emit(0, f[0]);
 #pragma unroll
     for (int p = 0; p < 9; ++p) {
-        const T cu = T(pair_cx(p)) * ux + T(pair_cy(p)) * uy + T(pair_cz(p)) * uz;
-        const T ce = T(pair_cx(p)) * ex + T(pair_cy(p)) * ey + T(pair_cz(p)) * ez;
+        const T cu = cdot<T>(p, ux, uy, uz);
+        const T ce = cdot<T>(p, ex, ey, ez);
         const T wr = w_pair<T>(p) * rho;
         const T s0 = a0 + T(4.5) * cu * cu;
         const T se = ae + T(4.5) * ce * ce;
@@ -98,7 +104,7 @@ __device__ __forceinline__ void equilibrium19(T (&f)[Q], T rho, T ux, T uy, T uz
     f[0] = w_rest<T>() * rho * a0;
 #pragma unroll
     for (int p = 0; p < 9; ++p) {
-        const T cu = T(pair_cx(p)) * ux + T(pair_cy(p)) * uy + T(pair_cz(p)) * uz;
+        const T cu = cdot<T>(p, ux, uy, uz);
         const T wr = w_pair<T>(p) * rho;
         const T s0 = a0 + T(4.5) * cu * cu;
         f[2 * p + 1] = wr * (s0 + T(3) * cu);

@@ -409,7 +409,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             uy = (om_r * jry + om_b * jby) * inv;
             uz = (om_r * jrz + om_b * jbz) * inv;
             // du^k = -G sum_i w_i rho^kbar(x+c_i) c_i (S2, S3, S6); a solid neighbour counts psi = 0 (S7)
-            T gx = zero, gy = zero, gz = zero;
+            T d[9];
 #pragma unroll
             for (int p = 0; p < 9; ++p) {
                 const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
@@ -419,11 +419,11 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                     if (lk >> (2 * p + 1) & 1u) vp = zero;
                     if (lk >> (2 * p + 2) & 1u) vm = zero;
                 }
-                const T d = w_pair<T>(p) * (vp - vm);
-                if (pair_cx(p)) gx += T(pair_cx(p)) * d;
-                if (pair_cy(p)) gy += T(pair_cy(p)) * d;
-                if (pair_cz(p)) gz += T(pair_cz(p)) * d;
+                d[p] = w_pair<T>(p) * (vp - vm);
             }
+            const T gx = (((d[0] + d[3]) + d[4]) + d[5]) + d[6];
+            const T gy = (((d[1] + d[3]) - d[4]) + d[7]) + d[8];
+            const T gz = (((d[2] + d[5]) - d[6]) + d[7]) - d[8];
             ex = ux - G * gx; ey = uy - G * gy; ez = uz - G * gz;
             // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) ----
             //      each value is stored (aligned, coalesced) as soon as it exists
