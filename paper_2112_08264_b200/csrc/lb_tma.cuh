@@ -61,6 +61,9 @@ __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* tm, int c0, i
     asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
                  ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+// plain global stores through a pointer the compiler must treat as opaque (see the running store pointer in the kernel)
+__device__ __forceinline__ void st_global(double* p, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
+__device__ __forceinline__ void st_global(float* p, float v) { asm volatile("st.global.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
 template <int ID, int COUNT>
 __device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(COUNT) : "memory"); }
 
@@ -428,7 +431,11 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) ----
             //      each value is stored (aligned, coalesced) as soon as it exists
             T* o = gk + zoff;                                               // values arrive in direction order: a running pointer
-            collide19_emit<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, [&](int, T v) { if (store_h) *o = v; o += NP; });
+            collide19_emit<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, [&](int, T v) {
+                if (store_h) st_global(o, v);
+                o += NP;
+                asm volatile("" : "+l"(o));                                // keep it a pointer: ptxas otherwise re-derives every address from scratch
+            });
         }
 
         // ---- density gather rho(y, t+1) = sum_i h_i(y - c_i): x by warp shuffles, z by register pipelines, y through
