@@ -64,6 +64,11 @@ __device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* tm, int c0, i
 // plain global stores through a pointer the compiler must treat as opaque (see the running store pointer in the kernel)
 __device__ __forceinline__ void st_global(double* p, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
 __device__ __forceinline__ void st_global(float* p, float v) { asm volatile("st.global.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
+// products and sums the compiler may not contract into an fma
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
 template <int ID, int COUNT>
 __device__ __forceinline__ void named_barrier() { asm volatile("bar.sync %0, %1;" ::"n"(ID), "n"(COUNT) : "memory"); }
 
@@ -323,7 +328,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const int btxm = btx == 0 ? ntx - 1 : btx - 1, btxp = btx == ntx - 1 ? 0 : btx + 1;
     const int btym = bty == 0 ? nty - 1 : bty - 1, btyp = bty == nty - 1 ? 0 : bty + 1;
     const T zero = T(0);
-    const T omc = T(1) - (k == 0 ? om_r : om_b);
+    const T om_own = k == 0 ? om_r : om_b, om_oth = k == 0 ? om_b : om_r;
+    const T omc = T(1) - om_own;
     const T* stage_k = stage + k * (9 * L::NA + 10 * L::WA);
     const T* hk = h + (long long)k * Q * NP;
     T* gk = g + (long long)k * Q * NP + own_xy;
@@ -403,14 +409,13 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         if (fluid) {
             const T* other = xm + ((1 - k) * NT + tl) * 4;
             const T orho = other[0], ojx = other[1], ojy = other[2], ojz = other[3];
-            const T rr = k == 0 ? rho : orho, rb = k == 0 ? orho : rho;
-            const T jrx = k == 0 ? jx : ojx, jry = k == 0 ? jy : ojy, jrz = k == 0 ? jz : ojz;
-            const T jbx = k == 0 ? ojx : jx, jby = k == 0 ? ojy : jy, jbz = k == 0 ? ojz : jz;
-            const T den = om_r * rr + om_b * rb;                            // common velocity (S4)
+            // common velocity (S4): u' = (om_r j^r + om_b j^b) / (om_r rho^r + om_b rho^b).  Both threads of the node must
+            // get the same bits: separately rounded products and one sum are commutative, a contracted fma is not.
+            const T den = add_rn(mul_rn(om_own, rho), mul_rn(om_oth, orho));
             const T inv = den != zero ? T(1) / den : zero;
-            ux = (om_r * jrx + om_b * jbx) * inv;
-            uy = (om_r * jry + om_b * jby) * inv;
-            uz = (om_r * jrz + om_b * jbz) * inv;
+            ux = add_rn(mul_rn(om_own, jx), mul_rn(om_oth, ojx)) * inv;
+            uy = add_rn(mul_rn(om_own, jy), mul_rn(om_oth, ojy)) * inv;
+            uz = add_rn(mul_rn(om_own, jz), mul_rn(om_oth, ojz)) * inv;
             // du^k = -G sum_i w_i rho^kbar(x+c_i) c_i (S2, S3, S6); a solid neighbour counts psi = 0 (S7)
             T d[9];
 #pragma unroll
