@@ -49,7 +49,8 @@ struct lb_ctx {
     int kernel;        // resolved LB_KERNEL_*
     int kernel_req;
     int zc;            // planes per CTA of the one-pass kernel
-    int zc_tma;        // ... of the TMA kernel (one CTA per SM)
+    int zc_tma;        // ... of the TMA kernel
+    int tma_ty;        // tile height of the TMA kernel: 8 (one CTA per SM) or 4 (two)
     CUtensorMap tmap[2][3];   // [buffer][narrow box 32 x TY, wide box (32 + 16 B) x TY, wrapped-column box 16 B x TY] over [k*19+i][z][y][x]
     bool have_tmap;
     double* stage;     // device staging, STAGE_NODES * 5 doubles
@@ -536,7 +537,7 @@ bool make_tmaps(lb_ctx* c) {
     for (int b = 0; b < 2; ++b)
         for (int w = 0; w < 3; ++w) {
             const cuuint32_t pad = cuuint32_t(16 / int(es));
-            const cuuint32_t box[4] = {w == 0 ? cuuint32_t(OP_TX) : (w == 1 ? OP_TX + pad : pad), cuuint32_t(OP_TY), 1, 1};
+            const cuuint32_t box[4] = {w == 0 ? cuuint32_t(OP_TX) : (w == 1 ? OP_TX + pad : pad), cuuint32_t(c->tma_ty), 1, 1};
             if (enc(&c->tmap[b][w], dt, 4, c->f[b], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
                 return false;
@@ -544,18 +545,18 @@ bool make_tmaps(lb_ctx* c) {
     return true;
 }
 
-template <typename T, bool HAS_SOLID>
+template <typename T, bool HAS_SOLID, int TY>
 int launch_tma(lb_ctx* c) {
-    auto kern = k_step_tma<T, HAS_SOLID, OP_TY>;
-    constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
+    auto kern = k_step_tma<T, HAS_SOLID, TY>;
+    constexpr size_t smem = TmaLayout<T, TY>::BYTES;
     static bool configured = false;                         // per instantiation
     if (!configured) {
         CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
         configured = true;
     }
-    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
+    const dim3 grid(c->nx / OP_TX, c->ny / TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
+    kern<<<grid, 2 * OP_TX * TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                         static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                         rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
                                                         c->zc_tma, om_r, om_b, G);
@@ -568,7 +569,8 @@ template <typename T>
 int step_tma(lb_ctx* c) {
     int rc = ensure_rho<T>(c);
     if (rc != LB_OK) return rc;
-    rc = c->has_solid ? launch_tma<T, true>(c) : launch_tma<T, false>(c);
+    if (c->tma_ty == 4) rc = c->has_solid ? launch_tma<T, true, 4>(c) : launch_tma<T, false, 4>(c);
+    else rc = c->has_solid ? launch_tma<T, true, 8>(c) : launch_tma<T, false, 8>(c);
     if (rc != LB_OK) return rc;
     c->cur ^= 1;
     c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
@@ -581,7 +583,8 @@ int tma_zc(const lb_ctx* c) {
     if (const char* e = std::getenv("LB_ONEPASS_ZC")) { const int v = std::atoi(e); if (v >= 1) return v < c->nz ? v : c->nz; }
     int dev = 0, sms = 148;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const double tiles = double(c->nx / OP_TX) * (c->ny / OP_TY);
+    const double tiles = double(c->nx / OP_TX) * (c->ny / c->tma_ty);
+    if (c->tma_ty == 4) sms *= 2;
     int best = c->nz;
     double best_cost = 1e300;
     for (int zc = 1; zc <= c->nz; ++zc) {
@@ -654,8 +657,8 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     ok = ok && cudaMalloc(&c->f[1], fbytes) == cudaSuccess;
     for (int r = 0; r < 2; ++r) ok = ok && cudaMalloc(&c->rho_in[r], size_t(2) * c->NP * es) == cudaSuccess;
     if (onepass_ok(c)) {
-        const long long ntx = nx / OP_TX, nty = ny / OP_TY;
-        c->s_x = round64((long long)nz * nty * ntx * 2 * OP_TY);
+        const long long ntx = nx / OP_TX, nty = ny / 4;    // sized for the smallest tile height any kernel uses
+        c->s_x = round64((long long)nz * nty * ntx * 2 * 4);
         c->s_y = round64((long long)nz * nty * 2 * nx);
         c->s_xy = round64((long long)nz * nty * ntx * 4);
         for (int r = 0; r < 2; ++r) {
@@ -679,6 +682,8 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
         lb_destroy(c);
         return nullptr;                                  // LB_ENOMEM
     }
+    c->tma_ty = 8;
+    if (const char* e = std::getenv("LB_TMA_TY")) { if (std::atoi(e) == 4) c->tma_ty = 4; }
     c->have_tmap = onepass_ok(c) && make_tmaps(c);
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
@@ -716,6 +721,7 @@ int lb_set_kernel(lb_ctx* c, int kind) {
     if (kind != LB_KERNEL_AUTO && kind != LB_KERNEL_TWOPASS && kind != LB_KERNEL_ONEPASS && kind != LB_KERNEL_TMA) return fail(LB_EINVAL, "unknown kernel kind");
     const int r = resolve_kernel(c, kind);
     if (r < 0) return fail(LB_EINVAL, "box shape does not allow this kernel");
+    if (r != c->kernel) c->rho_valid = false;               // the density edge arrays are laid out per tile shape
     c->kernel_req = kind;
     c->kernel = r;
     return LB_OK;

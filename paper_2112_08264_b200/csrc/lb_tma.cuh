@@ -81,9 +81,8 @@ struct TmaLayout {
     static constexpr int RW = TX + 2, RH = TY + 2, RS = RW * RH;       // density ring plane: tile + one-node frame
     static constexpr int SUP = TY * RW;                                // one y-stage plane: tile rows with an x frame
     __host__ __device__ static constexpr int align128(int elems) { return (elems * int(sizeof(T)) + 127) / 128 * 128 / int(sizeof(T)); }
-    static constexpr int XC = W * TY;                                  // offset of the wrapped-column box inside a wide slot
-    static constexpr int NA = align128(NT), WA = align128((W + PADX) * TY);   // slot sizes: narrow (c_x = 0) and wide (+ wrapped column), 128-byte multiples
-    static_assert((XC * sizeof(T)) % 128 == 0, "the wrapped-column box must start 128-byte aligned");
+    static constexpr int XC = align128(W * TY);                        // offset of the wrapped-column box inside a wide slot (128-byte aligned)
+    static constexpr int NA = align128(NT), WA = align128(XC + PADX * TY);    // slot sizes: narrow (c_x = 0) and wide (+ wrapped column), 128-byte multiples
     // number of wide slots before direction i (the directions with c_x != 0 are 1, 2, 7..14)
     __host__ __device__ static constexpr int wide_before(int i) { return (i > 1) + (i > 2) + (i > 7 ? (i - 7 < 8 ? i - 7 : 8) : 0); }
     __host__ __device__ static constexpr int slot_off(int q) {         // element offset of population plane q = k*19 + i
@@ -125,7 +124,7 @@ __device__ long long g_trace[64 * 16];
 // tile row and component) followed by one producer warp group (only its first warp works).  The producer
 // group gives its registers to the consumers (setmaxnreg), which is why it is a whole warp group.
 template <typename T, bool HAS_SOLID, int TY>
-__global__ void __launch_bounds__(2 * 32 * TY + 128, 1)
+__global__ void __launch_bounds__(2 * 32 * TY + 128, TY <= 4 ? 2 : 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
            const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
@@ -136,8 +135,9 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     static_assert(2 * L::NEX <= 96 && 2 * L::NEXY <= 96, "one ring thread per x / xy piece");
     static_assert(TY >= 2 && TY <= 8, "one named barrier per tile row (ids 1..TY)");
     // register hand-over between the warp groups: (2*NT + 128) threads start with 65536 / threads registers each
-    constexpr int START_REGS = (65536 / (NC + 128)) / 8 * 8;
-    constexpr int PRODUCER_REGS = 64;
+    constexpr int CTAS_PER_SM = TY <= 4 ? 2 : 1;
+    constexpr int START_REGS = (65536 / ((NC + 128) * CTAS_PER_SM)) / 8 * 8;
+    constexpr int PRODUCER_REGS = TY <= 4 ? 32 : 64;
     constexpr int CONSUMER_REGS = (START_REGS + (START_REGS - PRODUCER_REGS) * 128 / NC) / 8 * 8;
     extern __shared__ __align__(1024) unsigned char smem_tma[];
     T* sm = reinterpret_cast<T*>(smem_tma);
