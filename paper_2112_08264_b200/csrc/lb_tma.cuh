@@ -24,8 +24,9 @@
 //     64-thread named barrier per tile row; the y stage of the density gather is double-buffered behind
 //     one split-phase mbarrier per plane (arrive, independent stores, wait); the stage hand-off is
 //     mbarriers only;
-//   * the producer warp group gives most of its registers to the consumers (setmaxnreg): 16 consumer
-//     warps at 112 registers.
+//   * three more warps of the producer group assemble the density ring two planes ahead of its use;
+//   * the producer warp group hands registers to the consumers (setmaxnreg): 16 consumer warps at 104
+//     registers, producer group at 64.
 #pragma once
 #include <cuda.h>
 
