@@ -244,6 +244,45 @@ def test_full_size_sampled_outputs_and_invariants(oracle_mod, cfg_idx, dtype, to
             assert np.abs(m1 / m0 - 1).max() < 1e-5
 
 
+def test_headline_512_cube_sampled_moments_and_invariants(oracle_mod):
+    """Config 2 (512^3 fp64, the workload bench.py times by default, same kernel and launch configuration).
+    The 38 x 1 GiB populations are not brought to the host: rho_r, rho_b, u (Eq. 6-7, which sum all 38 of them)
+    are compared at sampled nodes with the oracle run on a cut-out of the SAME seeded initial fields, and the
+    conserved sums are followed over more steps."""
+    import torch
+    cfg = w.CONFIGS[2]
+    nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
+    need = 2 * 38 * cfg.n_nodes * 8 + 64 * cfg.n_nodes
+    if torch.cuda.mem_get_info()[0] < need:
+        pytest.skip("not enough free device memory for 512^3 fp64")
+    s, hw = 3, 7
+    rr, rb = cfg.fields()
+    R, Bl = rr.reshape(nz, ny, nx), rb.reshape(nz, ny, nx)
+    with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G) as box:
+        assert B.lb_kernel_name(box.h) == "tma"
+        box.set_fields(rr, rb)
+        m0, p0 = box.get_diagnostics()
+        box.step(s)
+        got = [a.reshape(nz, ny, nx) for a in box.get_moments()]
+        for (x, y, z) in _sample_points(nx, ny, nz, k=16):
+            ix = np.arange(x - hw, x + hw + 1) % nx
+            iy = np.arange(y - hw, y + hw + 1) % ny
+            iz = np.arange(z - hw, z + hw + 1) % nz
+            sub = np.ix_(iz, iy, ix)
+            L = 2 * hw + 1
+            o = oracle_mod.Oracle(L, L, L, cfg.tau_r, cfg.tau_b, cfg.G)
+            o.set_fields(R[sub].reshape(-1), Bl[sub].reshape(-1))
+            o.step(s)
+            want = [a.reshape(L, L, L)[hw, hw, hw] for a in o.get_moments()]
+            for gq, wq, scale in zip(got, want, (1.0, 1.0, 1e-3, 1e-3, 1e-3)):
+                assert abs(gq[z, y, x] - wq) < 1e-13 * scale + 1e-15, (x, y, z)
+        del got
+        box.step(17)
+        m1, p1 = box.get_diagnostics()
+        assert np.abs(m1 / m0 - 1).max() < 1e-13                 # per-component mass
+        assert np.abs(p1 - p0).max() < 1e-7                       # total momentum (|P| ~ 0, N = 1.3e8)
+
+
 # ---------------------------------------------------------------------------------------------
 # API behaviour on the device
 # ---------------------------------------------------------------------------------------------
