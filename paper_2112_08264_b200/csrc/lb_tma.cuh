@@ -24,9 +24,8 @@
 //     64-thread named barrier per tile row; the y stage of the density gather is double-buffered behind
 //     one split-phase mbarrier per plane (arrive, independent stores, wait); the stage hand-off is
 //     mbarriers only;
-//   * three more warps of the producer group assemble the density ring two planes ahead of its use;
-//   * the producer warp group hands registers to the consumers (setmaxnreg): 16 consumer warps at 104
-//     registers, producer group at 64.
+//   * the producer warp group gives most of its registers to the consumers (setmaxnreg): 16 consumer
+//     warps at 112 registers.
 #pragma once
 #include <cuda.h>
 
@@ -93,9 +92,8 @@ struct TmaLayout {
     static constexpr int STAGE_ELEMS = slot_off(NPOP);
     static constexpr unsigned STAGE_TX_BYTES = unsigned(2 * (9 * NT + 10 * W * TY) * sizeof(T));   // bytes the 38 boxes deliver
     static constexpr unsigned XCOL_TX_BYTES = unsigned(2 * 5 * PADX * TY * sizeof(T));             // ... plus the 10 wrapped-column boxes of one x side
-    static constexpr int NRING = 5;                                    // ring slots: planes z-1, z, z+1 in use, two more being prepared
-    static constexpr int RING = STAGE + STAGE_ELEMS;                   // [NRING][2][RS]  rho(t)
-    static constexpr int SU = RING + NRING * 2 * RS;                           // [2][2][2][SUP]  double-buffered z-summed Up, Um per component
+    static constexpr int RING = STAGE + STAGE_ELEMS;                   // [4][2][RS]      rho(t), planes z-1..z+2
+    static constexpr int SU = RING + 8 * RS;                           // [2][2][2][SUP]  double-buffered z-summed Up, Um per component
     static constexpr int XM = SU + 8 * SUP;                           // [2][NT][4]      rho^k, j^k of every node, exchanged between the two components' threads
     // ring pieces: every ring position has an `in` piece; the positions in the 4 columns / 4 rows next to a tile edge
     // also have an x / y piece, the 16 where they cross an xy piece
@@ -149,10 +147,9 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     T* xm = sm + L::XM;
     unsigned long long* bars = reinterpret_cast<unsigned long long*>(smem_tma + L::BAR_BYTE_OFF);
     unsigned long long* full = bars;          // the 38 boxes of the next plane have landed (tx bytes)
-    unsigned long long* done = bars + 6;      // [2] every consumer warp has copied its part of the stage of iteration `it` into registers: done[it & 1].
-                                              //     Alternating, because the ring warps may be two iterations behind the consumers
+    unsigned long long* done = bars + 2;      // every consumer warp has copied its part of the stage into registers
     unsigned long long* pub = bars + 3;       // every consumer warp has published its y-stage inputs of this plane
-    unsigned long long* rdy = bars + 4;       // [2] the ring warps have assembled the density ring plane iteration `it` needs: event `it` on rdy[it & 1]
+    unsigned long long* rdy = bars + 4;       // the producer warp has assembled the density ring plane this iteration needs
     int* tab = reinterpret_cast<int*>(smem_tma + L::TAB_BYTE_OFF);
 
     const int t = threadIdx.x;
@@ -170,10 +167,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     if (t == 0) {
         mbar_init(full, 1);
         mbar_init(done, 2 * TY);
-        mbar_init(done + 1, 2 * TY);
         mbar_init(pub, 2 * TY);
         mbar_init(rdy, 3);
-        mbar_init(rdy + 1, 3);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // ---- density ring bookkeeping: ring position pos (tile + one-node frame) of either component is the sum
@@ -246,7 +241,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                 TRACE(r == 0, rp - 2, 14);
                 ring_sync();                                               // every ring thread's pieces are in
                 TRACE(r == 0, rp - 2, 15);
-                T* dst = ring + (rp % L::NRING) * 2 * RS;
+                T* dst = ring + (rp & 3) * 2 * RS;
 #pragma unroll
                 for (int kk = 0; kk < 2; ++kk)
                     for (int pos = r; pos < RS; pos += NR) {
@@ -263,25 +258,21 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                 TRACE(r == 0, rp - 2, 11);
                 ring_sync();                                               // the landing slots may be overwritten
             };
-            // Ring plane rp (box plane z0 - 2 + rp) is needed from iteration rp - 2 on.  Event e (iteration e may read the
-            // ring) is signalled on rdy[e & 1]; the ring warps run one plane ahead of that: event 0 = planes 0..2, event
-            // j + 1 = plane j + 3, assembled in ring iteration j into the slot of plane j - 2, which every consumer warp had
-            // left when it arrived on done(j - 1).  Alternating barriers keep every waiter within one phase of its barrier.
-            for (int rp = 0; rp < 3; ++rp) {
+            for (int rp = 0; rp < 2; ++rp) {                                // iteration 0 needs ring planes 0, 1, 2
                 ring_fetch(rp);
                 ring_assemble(rp);
             }
-            __syncwarp();
-            if ((r & 31) == 0) mbar_arrive(rdy);
-            ring_fetch(3);
-            for (int j = 0; j + 1 < niter; ++j) {
-                if (j > 0) mbar_wait(done + ((j - 1) & 1), ((j - 1) >> 1) & 1);
+            ring_fetch(2);
+            for (int j = 0; j < niter; ++j) {
+                // ring plane j+2 (the z+1 neighbour plane of iteration j): its slot held plane j-2, last read in iteration
+                // j-2, which every consumer warp had left when it arrived on done(j-1)
+                if (j > 0) mbar_wait(done, (j - 1) & 1);
                 TRACE(r == 0, j, 8);
-                ring_assemble(j + 3);
+                ring_assemble(j + 2);
                 __syncwarp();
-                if ((r & 31) == 0) mbar_arrive(rdy + ((j + 1) & 1));
+                if ((r & 31) == 0) mbar_arrive(rdy);
                 TRACE(r == 0, j, 9);
-                if (j + 4 <= niter + 1) ring_fetch(j + 4);
+                if (j + 3 <= niter + 1) ring_fetch(j + 3);
                 TRACE(r == 0, j, 10);
             }
             return;
@@ -292,7 +283,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             const int z = z0 - 1 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
             if (lane == 0) {
-                if (j > 0) mbar_wait(done + ((j - 1) & 1), ((j - 1) >> 1) & 1);
+                if (j > 0) mbar_wait(done, (j - 1) & 1);
                 TRACE(true, j, 12);
                 mbar_expect_tx(full, L::STAGE_TX_BYTES + (wrap_xlo ? L::XCOL_TX_BYTES : 0u) + (wrap_xhi ? L::XCOL_TX_BYTES : 0u));
 #pragma unroll
@@ -368,8 +359,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         const long long zoff = (long long)zl * pl;
         const bool store_h = it >= 1 && it <= niter - 2;
         const bool store_rho = it >= 2;                 // target plane z-1 lies in [z0, z1)
-        const int s0 = (it + 1) % L::NRING;             // ring slots of planes z, z-1, z+1
-        const int s_lo = it % L::NRING, s_hi = (it + 2) % L::NRING;
+        const int s0 = (it + 1) & 3;                    // ring slot of plane z
         const bool fluid = !HAS_SOLID || !(lk & OP_SOLID_BIT);   // nothing happens inside a particle
         T* SU = SUk + (it & 1) * 4 * SUP;
 
@@ -377,8 +367,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         TRACE(t == 0, it, 0);
         mbar_wait(full, it & 1);
         TRACE(t == 0, it, 1);
-        mbar_wait(rdy + (it & 1), (it >> 1) & 1);       // density ring planes z-1, z, z+1 are in place (waited for before the
-                                                        // arrival on `done`, which is what lets the ring warps go on)
+        mbar_wait(rdy, it & 1);                         // density ring planes z-1, z, z+1 are in place (before `done`: the producer
+                                                        // must not get two phases ahead of any waiter)
         TRACE(t == 0, it, 2);
         T f[Q];
 #pragma unroll
@@ -401,7 +391,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         }
         __syncwarp();
         TRACE(t == 0, it, 3);
-        if (lane_lo) mbar_arrive(done + (it & 1));      // the producer may refill the stage with the next plane
+        if (lane_lo) mbar_arrive(done);                 // the producer may refill the stage with the next plane
 
         // ---- moments of this component (Eq. 6-7), exchanged with the other component's thread of the same node ----
         T rho = zero, jx = zero, jy = zero, jz = zero;
@@ -430,7 +420,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             T d[9];
 #pragma unroll
             for (int p = 0; p < 9; ++p) {
-                const int sp = pair_cz(p) == 0 ? s0 : (pair_cz(p) > 0 ? s_hi : s_lo), sm_ = pair_cz(p) == 0 ? s0 : (pair_cz(p) > 0 ? s_lo : s_hi);
+                const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
                 T vp = ring_o[sp * 2 * RS + own_r + pair_cy(p) * RW + pair_cx(p)];
                 T vm = ring_o[sm_ * 2 * RS + own_r - pair_cy(p) * RW - pair_cx(p)];
                 if (HAS_SOLID) {
