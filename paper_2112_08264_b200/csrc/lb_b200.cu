@@ -52,7 +52,6 @@ struct lb_ctx {
     int zc_tma;        // ... of the TMA kernel
     int tma_ty;        // tile height of the TMA kernel: 8 (one CTA per SM) or 4 (two)
     CUtensorMap tmap[2][3];   // [buffer][narrow box 32 x TY, wide box (32 + 16 B) x TY, wrapped-column box 16 B x TY] over [k*19+i][z][y][x]
-    CUtensorMap tmap_rho[2];  // [rho buffer] window (32 + 32 B) x (TY + 2) over rho_in[k][z][y][x]
     bool have_tmap;
     double* stage;     // device staging, STAGE_NODES * 5 doubles
     double* diag_part; // [DIAG_BLOCKS][5]
@@ -543,12 +542,6 @@ bool make_tmaps(lb_ctx* c) {
                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
                 return false;
         }
-    const cuuint64_t rdim[4] = {cuuint64_t(c->nx), cuuint64_t(c->ny), cuuint64_t(c->nz), 2};
-    const cuuint32_t rbox[4] = {cuuint32_t(OP_TX + 2 * (16 / int(es))), cuuint32_t(c->tma_ty + 2), 1, 1};
-    for (int r = 0; r < 2; ++r)
-        if (enc(&c->tmap_rho[r], dt, 4, c->rho_in[r], rdim, gstr, rbox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-                CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-            return false;
     return true;
 }
 
@@ -563,7 +556,7 @@ int launch_tma(lb_ctx* c) {
     }
     const dim3 grid(c->nx / OP_TX, c->ny / TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    kern<<<grid, 2 * OP_TX * TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], c->tmap_rho[c->rcur], static_cast<const T*>(c->f[c->cur]),
+    kern<<<grid, 2 * OP_TX * TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                         static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                         rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
                                                         c->zc_tma, om_r, om_b, G);

@@ -24,8 +24,8 @@
 //     64-thread named barrier per tile row; the y stage of the density gather is double-buffered behind
 //     one split-phase mbarrier per plane (arrive, independent stores, wait); the stage hand-off is
 //     mbarriers only;
-//   * three more warps of the producer group assemble the density ring two planes ahead of its use: the rho_in window
-//     of the tile and its frame by TMA straight into the ring slot, the edge pieces from tabulated lists;
+//   * three more warps of the producer group assemble the density ring two planes ahead of its use from tabulated
+//     piece lists (cp.async into landing slots, then the fixed-order sums);
 //   * the producer warp group hands registers to the consumers (setmaxnreg): 16 consumer warps at 104
 //     registers, producer group at 64.
 #pragma once
@@ -52,16 +52,6 @@ __device__ __forceinline__ void mbar_wait(void* bar, unsigned parity) {
         "{\n\t.reg .pred P1;\n\tLAB_WAIT:\n\t"
         "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1, 0x989680;\n\t"
         "@P1 bra DONE;\n\tbra LAB_WAIT;\n\tDONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// the same for a waiter that is in no hurry (the ring warps): poll rarely, sleep in between
-__device__ __forceinline__ void mbar_wait_relaxed(void* bar, unsigned parity) {
-    for (;;) {
-        unsigned ok;
-        asm volatile("{\n\t.reg .pred P1;\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\tselp.b32 %0, 1, 0, P1;\n\t}"
-                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-        if (ok) break;
-        __nanosleep(400);
-    }
 }
 // box load: coordinates (x, y, z, plane); x * sizeof(T) must be a multiple of 16 (see header)
 __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int c0, int c1, int c2, int c3) {
@@ -104,30 +94,22 @@ struct TmaLayout {
     static constexpr int STAGE_ELEMS = slot_off(NPOP);
     static constexpr unsigned STAGE_TX_BYTES = unsigned(2 * (9 * NT + 10 * W * TY) * sizeof(T));   // bytes the 38 boxes deliver
     static constexpr unsigned XCOL_TX_BYTES = unsigned(2 * 5 * PADX * TY * sizeof(T));             // ... plus the 10 wrapped-column boxes of one x side
-    // density ring: per slot and component one TMA window of rho_in, RH rows of RWP = TX + 2*PADX elements starting at
-    // x0 - PADX (16-byte aligned); ring position (rx, ry) of the tile frame sits at (ry + 1) * RWP + rx + PADX
-    static constexpr int RWP = TX + 2 * PADX, RSP = align128(RWP * RH);
-    static constexpr int RING = STAGE + STAGE_ELEMS;                   // [4][2][RSP]     rho(t), planes z-1..z+2
-    static constexpr int SU = RING + 8 * RSP;                          // [2][2][2][SUP]  double-buffered z-summed Up, Um per component
-    static constexpr int XM = SU + 8 * SUP;                            // [2][NT][4]      rho^k, j^k of every node, exchanged between the two components' threads
-    // ring pieces besides the TMA window: the ring positions in the 4 columns / 4 rows next to a tile edge also have an
-    // x / y piece, the 16 where they cross an xy piece; in tiles at the box boundary the frame positions beyond it have
-    // their rho_in value fetched from the wrapped node
-    static constexpr int NIW = 2 * RH + 2 * RW, NEX = 4 * RH, NEY = 4 * RW, NEXY = 16;
-    static constexpr int NEDGE = 4 * RH + 4 * (RW - 4);                // ring positions that have any of these pieces
-    static constexpr int NPIECE = 2 * (NIW + NEX + NEY + NEXY);        // landing slots (cp.async), both components: [inw][x][y][xy]
-    static constexpr int RP = XM + 8 * NT;
-    static constexpr int END = RP + NPIECE;
+    static constexpr int RING = STAGE + STAGE_ELEMS;                   // [4][2][RS]      rho(t), planes z-1..z+2
+    static constexpr int SU = RING + 8 * RS;                           // [2][2][2][SUP]  double-buffered z-summed Up, Um per component
+    static constexpr int XM = SU + 8 * SUP;                           // [2][NT][4]      rho^k, j^k of every node, exchanged between the two components' threads
+    // ring pieces: every ring position has an `in` piece; the positions in the 4 columns / 4 rows next to a tile edge
+    // also have an x / y piece, the 16 where they cross an xy piece
+    static constexpr int NEX = 4 * RH, NEY = 4 * RW, NEXY = 16;
+    static constexpr int RP_IN = XM + 8 * NT;                          // [2][RS]    landing slots of the pieces (cp.async), per component
+    static constexpr int RP_X = RP_IN + 2 * RS;                        // [2][NEX]
+    static constexpr int RP_Y = RP_X + 2 * NEX;                        // [2][NEY]
+    static constexpr int RP_XY = RP_Y + 2 * NEY;                       // [2][NEXY]
+    static constexpr int END = RP_XY + 2 * NEXY;
     static constexpr size_t TAB_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
-    // tables of the ring warps, built once per CTA.  int T_SRC[NPIECE]: element offset of piece e inside one plane of its
-    // array (-1 = not needed in this tile); int T_EPOS[NEDGE]: ring index of edge position m; int T_EPK[NEDGE]: list
-    // indices of its pieces (inw | x << 8 | y << 16 | xy << 24, 255 = none); byte T_CLS[NPIECE]: array and component
-    // (piece * 2 + k); u64 RB[8]: byte address of plane 0 of (array, component); u64 PS[4]: plane strides in bytes;
-    // u64 ZB[8]: RB advanced to the plane being fetched
-    static constexpr int T_SRC = 0, T_EPOS = NPIECE, T_EPK = NPIECE + NEDGE, T_INTS = NPIECE + 2 * NEDGE;
-    static constexpr size_t CLS_BYTE_OFF = TAB_BYTE_OFF + size_t(T_INTS) * sizeof(int);
-    static constexpr size_t RB_BYTE_OFF = (CLS_BYTE_OFF + NPIECE + 15) / 16 * 16;
-    static constexpr size_t BAR_BYTE_OFF = RB_BYTE_OFF + 20 * sizeof(unsigned long long);
+    // int tables: T_IN[RS] offset of the in piece inside a plane; T_PK[RS] packed list indices (x | y << 8 | xy << 16, 255 = none);
+    // T_X[NEX], T_Y[NEY], T_XY[NEXY] offsets of the edge pieces inside their arrays' planes
+    static constexpr int T_IN = 0, T_PK = RS, T_X = 2 * RS, T_Y = T_X + NEX, T_XY = T_Y + NEY, T_END = T_XY + NEXY;
+    static constexpr size_t BAR_BYTE_OFF = (TAB_BYTE_OFF + size_t(T_END) * sizeof(int) + 15) / 16 * 16;
     static constexpr size_t BYTES = BAR_BYTE_OFF + 8 * sizeof(unsigned long long);
 };
 
@@ -146,12 +128,13 @@ __device__ long long g_trace[64 * 16];
 template <typename T, bool HAS_SOLID, int TY>
 __global__ void __launch_bounds__(2 * 32 * TY + 128, TY <= 4 ? 2 : 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
-           const __grid_constant__ CUtensorMap tm_c, const __grid_constant__ CUtensorMap tm_rho, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
+           const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
            T om_r, T om_b, T G) {
     using L = TmaLayout<T, TY>;
-    constexpr int TX = L::TX, NT = L::NT, NC = 2 * NT, RW = L::RW, RH = L::RH, RWP = L::RWP, RSP = L::RSP, SUP = L::SUP, W = L::W, PADX = L::PADX;
-    static_assert(L::NIW < 255 && L::NEY < 255, "piece list indices are packed into bytes");
+    constexpr int TX = L::TX, NT = L::NT, NC = 2 * NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
+    static_assert(RS <= 2 * NT, "ring fill: at most two positions per consumer thread");
+    static_assert(2 * L::NEX <= 96 && 2 * L::NEXY <= 96, "one ring thread per x / xy piece");
     static_assert(TY >= 2 && TY <= 8, "one named barrier per tile row (ids 1..TY)");
     // register hand-over between the warp groups: (2*NT + 128) threads start with 65536 / threads registers each
     constexpr int CTAS_PER_SM = TY <= 4 ? 2 : 1;
@@ -168,7 +151,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     unsigned long long* full = bars;          // the 38 boxes of the next plane have landed (tx bytes)
     unsigned long long* done = bars + 2;      // every consumer warp has copied its part of the stage into registers
     unsigned long long* pub = bars + 3;       // every consumer warp has published its y-stage inputs of this plane
-    unsigned long long* rfull = bars + 1;     // the TMA window of the ring plane being assembled has landed
     unsigned long long* rdy = bars + 4;       // the producer warp has assembled the density ring plane this iteration needs
     int* tab = reinterpret_cast<int*>(smem_tma + L::TAB_BYTE_OFF);
 
@@ -189,74 +171,36 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         mbar_init(done, 2 * TY);
         mbar_init(pub, 2 * TY);
         mbar_init(rdy, 3);
-        mbar_init(rfull, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    // ---- density ring bookkeeping (lb_onepass.cuh): the density of ring position (rx, ry) is ((in + x) + y) + xy.  The
-    //      `in` values of the whole frame come as one TMA window per component; the x / y / xy pieces of the positions
-    //      next to a tile edge, and the `in` values the window cannot reach in a tile at the box boundary (the TMA does
-    //      not wrap), come by cp.async from lists tabulated here once ----
-    unsigned char* cls = smem_tma + L::CLS_BYTE_OFF;
-    unsigned long long* rb = reinterpret_cast<unsigned long long*>(smem_tma + L::RB_BYTE_OFF);   // RB[8], PS[4], ZB[8]
-    {
+    // ---- density ring bookkeeping: ring position pos (tile + one-node frame) of either component is the sum
+    //      ((in + x) + y) + xy of up to four single-writer pieces (lb_onepass.cuh); where they live, tabulated once ----
+    for (int pos = t; pos < RS; pos += blockDim.x) {
+        const int rx = pos % RW - 1, ry = pos / RW - 1;
         const int txm = btx == 0 ? ntx - 1 : btx - 1, txp = btx == ntx - 1 ? 0 : btx + 1;
         const int tym = bty == 0 ? nty - 1 : bty - 1, typ = bty == nty - 1 ? 0 : bty + 1;
-        auto edge = [&](int q, int n) { return q == 0 ? -1 : (q == 1 ? 0 : (q == 2 ? n - 1 : n)); };   // the 4 columns / rows at a tile edge
-        auto edge_of = [&](int c, int n) { return c == -1 ? 0 : (c == 0 ? 1 : (c == n - 1 ? 2 : (c == n ? 3 : -1))); };
-        // does the frame position leave the box in x / in y?
-        auto xwrap = [&](int rx) { return (rx < 0 && btx == 0) || (rx >= TX && btx == ntx - 1); };
-        auto ywrap = [&](int ry) { return (ry < 0 && bty == 0) || (ry >= TY && bty == nty - 1); };
-        // list index of the wrapped `in` piece of (rx, ry): the column lists first (rx = -1, TX), then the row lists
-        auto inw_index = [&](int rx, int ry) { return xwrap(rx) ? (rx < 0 ? 0 : 1) * RH + ry + 1 : 2 * RH + (ry < 0 ? 0 : 1) * RW + rx + 1; };
-        for (int e = t; e < L::NPIECE; e += blockDim.x) {
-            int piece, m = e;                                               // list e -> (array, component, entry m) -> (rx, ry)
-            if (m < 2 * L::NIW) piece = 0;
-            else if ((m -= 2 * L::NIW) < 2 * L::NEX) piece = 1;
-            else if ((m -= 2 * L::NEX) < 2 * L::NEY) piece = 2;
-            else { m -= 2 * L::NEY; piece = 3; }
-            const int cnt = piece == 0 ? L::NIW : (piece == 1 ? L::NEX : (piece == 2 ? L::NEY : L::NEXY));
-            const int kk = m >= cnt;
-            m -= kk * cnt;
-            int rx, ry;
-            bool used = true;
-            if (piece == 0) {
-                if (m < 2 * RH) { rx = m < RH ? -1 : TX; ry = m % RH - 1; }
-                else { const int q = m - 2 * RH; ry = q < RW ? -1 : TY; rx = q % RW - 1; }
-                used = (xwrap(rx) || ywrap(ry)) && inw_index(rx, ry) == m;
-            } else if (piece == 1) { rx = edge(m / RH, TX); ry = m % RH - 1; }
-            else if (piece == 2) { ry = edge(m / RW, TY); rx = m % RW - 1; }
-            else { ry = edge(m / 4, TY); rx = edge(m % 4, TX); }
-            const int otx = rx < 0 ? txm : (rx >= TX ? txp : btx), oty = ry < 0 ? tym : (ry >= TY ? typ : bty);
-            const int lx = rx < 0 ? TX - 1 : (rx >= TX ? 0 : rx), ly = ry < 0 ? TY - 1 : (ry >= TY ? 0 : ry);
-            tab[L::T_SRC + e] = !used ? -1
-                              : piece == 0 ? (oty * TY + ly) * nx + otx * TX + lx
-                              : piece == 1 ? ((oty * ntx + otx) * 2 + (lx != 0)) * TY + ly
-                              : piece == 2 ? (oty * 2 + (ly != 0)) * nx + otx * TX + lx
-                                           : (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
-            cls[e] = (unsigned char)(piece * 2 + kk);
+        const int otx = rx < 0 ? txm : (rx >= TX ? txp : btx), oty = ry < 0 ? tym : (ry >= TY ? typ : bty);
+        const int lx = rx < 0 ? TX - 1 : (rx >= TX ? 0 : rx), ly = ry < 0 ? TY - 1 : (ry >= TY ? 0 : ry);
+        const int c4 = rx == -1 ? 0 : (rx == 0 ? 1 : (rx == TX - 1 ? 2 : (rx == TX ? 3 : -1)));   // edge column / row of the tile grid
+        const int r4 = ry == -1 ? 0 : (ry == 0 ? 1 : (ry == TY - 1 ? 2 : (ry == TY ? 3 : -1)));
+        tab[L::T_IN + pos] = (oty * TY + ly) * nx + otx * TX + lx;
+        int pk = 0xFFFFFF;
+        if (c4 >= 0) {
+            const int m = c4 * L::RH + ry + 1;
+            tab[L::T_X + m] = ((oty * ntx + otx) * 2 + (lx != 0)) * TY + ly;
+            pk = (pk & ~0xFF) | m;
         }
-        for (int m = t; m < L::NEDGE; m += blockDim.x) {                    // the frame positions that have pieces
-            int rx, ry;
-            if (m < 4 * RH) { rx = edge(m / RH, TX); ry = m % RH - 1; }
-            else { const int q = m - 4 * RH; ry = edge(q / (RW - 4), TY); rx = q % (RW - 4) + 1; }
-            const int c4 = edge_of(rx, TX), r4 = edge_of(ry, TY);
-            unsigned pk = 0xFFFFFFFFu;
-            if (xwrap(rx) || ywrap(ry)) pk = (pk & ~0xFFu) | unsigned(inw_index(rx, ry));
-            if (c4 >= 0) pk = (pk & ~0xFF00u) | (unsigned(c4 * RH + ry + 1) << 8);
-            if (r4 >= 0) pk = (pk & ~0xFF0000u) | (unsigned(r4 * RW + rx + 1) << 16);
-            if (c4 >= 0 && r4 >= 0) pk = (pk & ~0xFF000000u) | (unsigned(r4 * 4 + c4) << 24);
-            tab[L::T_EPOS + m] = (ry + 1) * RWP + rx + PADX;
-            tab[L::T_EPK + m] = int(pk);
+        if (r4 >= 0) {
+            const int m = r4 * RW + rx + 1;
+            tab[L::T_Y + m] = (oty * 2 + (ly != 0)) * nx + otx * TX + lx;
+            pk = (pk & ~0xFF00) | (m << 8);
         }
-        if (t < 8) {
-            const int piece = t >> 1, kk = t & 1;
-            const T* base = piece == 0 ? ri.in + kk * ri.s_in : (piece == 1 ? ri.x + kk * ri.s_x : (piece == 2 ? ri.y + kk * ri.s_y : ri.xy + kk * ri.s_xy));
-            rb[t] = reinterpret_cast<unsigned long long>(base);
+        if (c4 >= 0 && r4 >= 0) {
+            const int m = r4 * 4 + c4;
+            tab[L::T_XY + m] = (oty * ntx + otx) * 4 + (ly != 0) * 2 + (lx != 0);
+            pk = (pk & ~0xFF0000) | (m << 16);
         }
-        if (t < 4) {
-            const long long ps = t == 0 ? pl : (t == 1 ? (long long)nty * ntx * 2 * TY : (t == 2 ? (long long)nty * 2 * nx : (long long)nty * ntx * 4));
-            rb[8 + t] = (unsigned long long)ps * sizeof(T);
-        }
+        tab[L::T_PK + pos] = pk;
     }
     __syncthreads();
 
@@ -267,61 +211,66 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             // ---- ring warps (3): assemble the density ring, one plane per iteration, two planes ahead of its use ----
             const int r = t - NC - 32;
             constexpr int NR = 96;
-            T* scr = sm + L::RP;                                           // landing slots of the pieces: [inw][x][y][xy], two components each
+            const long long psx_ = (long long)nty * ntx * 2 * TY, psy_ = (long long)nty * 2 * nx, psxy_ = (long long)nty * ntx * 4;
+            T* s_in = sm + L::RP_IN;
+            T* s_x = sm + L::RP_X;
+            T* s_y = sm + L::RP_Y;
+            T* s_xy = sm + L::RP_XY;
             auto ring_sync = [&]() { asm volatile("bar.sync %0, %1;" ::"n"(TY + 2), "n"(NR) : "memory"); };
             // ask for the pieces of ring plane rp (= box plane z0 - 2 + rp): asynchronous, no registers in flight
             auto ring_fetch = [&](int rp) {
-                const int zp = wrapz(z0 - 2 + rp);
-                if (r < 8) rb[12 + r] = rb[r] + (unsigned long long)zp * rb[8 + (r >> 1)];
-                if (r == 8) {                                               // and its TMA windows into L2
-                    tma_prefetch_4d(&tm_rho, x0 - PADX, y0 - 1, zp, 0);
-                    tma_prefetch_4d(&tm_rho, x0 - PADX, y0 - 1, zp, 1);
+                const long long zp = wrapz(z0 - 2 + rp);
+#pragma unroll
+                for (int kk = 0; kk < 2; ++kk) {
+                    const T* b_in = ri.in + kk * ri.s_in + zp * pl;
+                    for (int pos = r; pos < RS; pos += NR) cp_async<sizeof(T)>(s_in + kk * RS + pos, b_in + tab[L::T_IN + pos]);
+                    const T* b_y = ri.y + kk * ri.s_y + zp * psy_;
+                    for (int m = r; m < L::NEY; m += NR) cp_async<sizeof(T)>(s_y + kk * L::NEY + m, b_y + tab[L::T_Y + m]);
                 }
-                ring_sync();
-                for (int e = r; e < L::NPIECE; e += NR) {
-                    const int off = tab[L::T_SRC + e];
-                    if (off >= 0) cp_async<sizeof(T)>(scr + e, reinterpret_cast<const T*>(rb[12 + cls[e]]) + off);
+                if (r < 2 * L::NEX) {
+                    const int kk = r >= L::NEX, m = r - kk * L::NEX;
+                    cp_async<sizeof(T)>(s_x + r, ri.x + kk * ri.s_x + zp * psx_ + tab[L::T_X + m]);
+                }
+                if (r >= NR - 2 * L::NEXY) {
+                    const int q = r - (NR - 2 * L::NEXY), kk = q >= L::NEXY, m = q - kk * L::NEXY;
+                    cp_async<sizeof(T)>(s_xy + q, ri.xy + kk * ri.s_xy + zp * psxy_ + tab[L::T_XY + m]);
                 }
                 cp_async_commit();
             };
-            // the `in` window lands in the ring slot itself; the positions next to a tile edge then add their pieces in the
-            // fixed order ((in + x) + y) + xy.  `nth` counts the planes assembled so far (the phase of rfull).
-            auto ring_assemble = [&](int rp, int nth) {
-                T* dst = ring + (rp & 3) * 2 * RSP;
-                if (r == 0) {
-                    const int zp = wrapz(z0 - 2 + rp);
-                    mbar_expect_tx(rfull, unsigned(2 * RWP * RH * sizeof(T)));
-                    tma_load_4d(dst, &tm_rho, rfull, x0 - PADX, y0 - 1, zp, 0);
-                    tma_load_4d(dst + RSP, &tm_rho, rfull, x0 - PADX, y0 - 1, zp, 1);
-                }
+            // ... and add them up in the fixed order ((in + x) + y) + xy once they have landed
+            auto ring_assemble = [&](int rp) {
                 cp_async_wait<0>();
+                TRACE(r == 0, rp - 2, 14);
                 ring_sync();                                               // every ring thread's pieces are in
-                mbar_wait(rfull, nth & 1);
-                for (int idx = r; idx < 2 * L::NEDGE; idx += NR) {
-                    const int kk = idx >= L::NEDGE, m = idx - kk * L::NEDGE;
-                    const unsigned pk = unsigned(tab[L::T_EPK + m]);
-                    const int pos = kk * RSP + tab[L::T_EPOS + m];
-                    const unsigned iw = pk & 255u, ix = (pk >> 8) & 255u, iy = (pk >> 16) & 255u, ixy = pk >> 24;
-                    T v = iw != 255u ? scr[kk * L::NIW + iw] : dst[pos];
-                    if (ix != 255u) v += scr[2 * L::NIW + kk * L::NEX + ix];
-                    if (iy != 255u) v += scr[2 * L::NIW + 2 * L::NEX + kk * L::NEY + iy];
-                    if (ixy != 255u) v += scr[2 * L::NIW + 2 * L::NEX + 2 * L::NEY + kk * L::NEXY + ixy];
-                    dst[pos] = v;
-                }
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // these writes before the slot's next TMA window
+                TRACE(r == 0, rp - 2, 15);
+                T* dst = ring + (rp & 3) * 2 * RS;
+#pragma unroll
+                for (int kk = 0; kk < 2; ++kk)
+                    for (int pos = r; pos < RS; pos += NR) {
+                        T v = s_in[kk * RS + pos];
+                        const int pk = tab[L::T_PK + pos];
+                        if (pk != 0xFFFFFF) {
+                            const int ix = pk & 255, iy = (pk >> 8) & 255, ixy = (pk >> 16) & 255;
+                            if (ix != 255) v += s_x[kk * L::NEX + ix];
+                            if (iy != 255) v += s_y[kk * L::NEY + iy];
+                            if (ixy != 255) v += s_xy[kk * L::NEXY + ixy];
+                        }
+                        dst[kk * RS + pos] = v;
+                    }
+                TRACE(r == 0, rp - 2, 11);
                 ring_sync();                                               // the landing slots may be overwritten
             };
             for (int rp = 0; rp < 2; ++rp) {                                // iteration 0 needs ring planes 0, 1, 2
                 ring_fetch(rp);
-                ring_assemble(rp, rp);
+                ring_assemble(rp);
             }
             ring_fetch(2);
             for (int j = 0; j < niter; ++j) {
                 // ring plane j+2 (the z+1 neighbour plane of iteration j): its slot held plane j-2, last read in iteration
                 // j-2, which every consumer warp had left when it arrived on done(j-1)
-                if (j > 0) mbar_wait_relaxed(done, (j - 1) & 1);
+                if (j > 0) mbar_wait(done, (j - 1) & 1);
                 TRACE(r == 0, j, 8);
-                ring_assemble(j + 2, j + 2);
+                ring_assemble(j + 2);
                 __syncwarp();
                 if ((r & 31) == 0) mbar_arrive(rdy);
                 TRACE(r == 0, j, 9);
@@ -375,7 +324,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const int tx = tl % TX, ty = tl / TX;
     const int x = x0 + tx, y = y0 + ty;
     const int own_xy = y * nx + x;
-    const int own_r = (ty + 1) * RWP + tx + PADX;                          // ring position (window of the tile + frame)
+    const int own_r = (ty + 1) * RW + tx + 1;                              // ring position (tile + frame)
     const int own_s = ty * RW + tx + 1;                                    // y-stage plane position (x frame only)
     const long long psx = (long long)nty * ntx * 2 * TY, psy = (long long)nty * 2 * nx, psxy = (long long)nty * ntx * 4;
     const int btxm = btx == 0 ? ntx - 1 : btx - 1, btxp = btx == ntx - 1 ? 0 : btx + 1;
@@ -386,7 +335,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const T* stage_k = stage + k * (9 * L::NA + 10 * L::WA);
     const T* hk = h + (long long)k * Q * NP;
     T* gk = g + (long long)k * Q * NP + own_xy;
-    const T* ring_o = ring + (1 - k) * RSP;                                // the OTHER component's density (S2)
+    const T* ring_o = ring + (1 - k) * RS;                                 // the OTHER component's density (S2)
     T* SUk = SUb + k * 2 * SUP;
     T* ro_in = ro.in + k * ro.s_in + own_xy;
     const bool lane_lo = tx == 0, lane_hi = tx == TX - 1, row_lo = ty == 0, row_hi = ty == TY - 1;
@@ -474,8 +423,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
 #pragma unroll
             for (int p = 0; p < 9; ++p) {
                 const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
-                T vp = ring_o[sp * 2 * RSP + own_r + pair_cy(p) * RWP + pair_cx(p)];
-                T vm = ring_o[sm_ * 2 * RSP + own_r - pair_cy(p) * RWP - pair_cx(p)];
+                T vp = ring_o[sp * 2 * RS + own_r + pair_cy(p) * RW + pair_cx(p)];
+                T vm = ring_o[sm_ * 2 * RS + own_r - pair_cy(p) * RW - pair_cx(p)];
                 if (HAS_SOLID) {
                     if (lk >> (2 * p + 1) & 1u) vp = zero;
                     if (lk >> (2 * p + 2) & 1u) vm = zero;
