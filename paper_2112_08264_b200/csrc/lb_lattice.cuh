@@ -97,6 +97,27 @@ __device__ __forceinline__ void collide19_emit(T (&f)[Q], T rho, T omc, T ux, T 
     }
 }
 
+// The same collision, handing the post-collision values to the caller pair by pair (`rest(h_0)`, then `pair(p, h_{2p+1},
+// h_{2p+2})` for p = 0..8) and keeping nothing: what the caller does with a pair (store, gather) interleaves with the
+// arithmetic of the next ones, and the inputs' registers die as the loop proceeds.
+template <typename T, typename Rest, typename Pair>
+__device__ __forceinline__ void collide19_pairs(const T (&f)[Q], T rho, T omc, T ux, T uy, T uz, T ex, T ey, T ez, Rest rest, Pair pair) {
+    const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    const T ae = T(1) - T(1.5) * (ex * ex + ey * ey + ez * ez);
+    rest(omc * f[0] + w_rest<T>() * rho * (ae - omc * a0));
+#pragma unroll
+    for (int p = 0; p < 9; ++p) {
+        const T cu = cdot<T>(p, ux, uy, uz);
+        const T ce = cdot<T>(p, ex, ey, ez);
+        const T wr = w_pair<T>(p) * rho;
+        const T s0 = a0 + T(4.5) * cu * cu;
+        const T se = ae + T(4.5) * ce * ce;
+        const T sym = wr * (se - omc * s0);
+        const T asym = (T(3) * wr) * (ce - omc * cu);
+        pair(p, omc * f[2 * p + 1] + (sym + asym), omc * f[2 * p + 2] + (sym - asym));
+    }
+}
+
 // Eq. 10 for all 19 directions.
 template <typename T>
 __device__ __forceinline__ void equilibrium19(T (&f)[Q], T rho, T ux, T uy, T uz) {

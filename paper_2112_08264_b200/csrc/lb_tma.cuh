@@ -435,64 +435,74 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             const T gy = (((d[1] + d[3]) - d[4]) + d[7]) + d[8];
             const T gz = (((d[2] + d[5]) - d[6]) + d[7]) - d[8];
             ex = ux - G * gx; ey = uy - G * gy; ez = uz - G * gz;
-            // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) ----
-            //      each value is stored (aligned, coalesced) as soon as it exists
-            T* o = gk + zoff;                                               // values arrive in direction order: a running pointer
-            collide19_emit<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, [&](int, T v) {
-                if (store_h) st_global(o, v);
-                o += NP;
-                asm volatile("" : "+l"(o));                                // keep it a pointer: ptxas otherwise re-derives every address from scratch
-            });
         }
 
-        // ---- density gather rho(y, t+1) = sum_i h_i(y - c_i): x by warp shuffles, z by register pipelines, y through
-        //      shared memory (two values per node) ----
-        T u0[3] = {zero, f[0], zero};                    // row sums by c_z, c_y = 0
+        // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5), and, pair by pair as the post-collision values
+        //      appear: their (aligned, coalesced) stores and the x stage of the density gather
+        //      rho(y, t+1) = sum_i h_i(y - c_i): x by warp shuffles, z by register pipelines, y through shared memory.
+        //      A solid node runs the same instructions on zeros (the shuffles need every lane) and stores nothing. ----
+        T u0[3] = {zero, zero, zero};                    // row sums by c_z, c_y = 0
         T ee[3] = {zero, zero, zero};                    // on lanes tx = 0 / TX-1: what leaves the tile in x with c_y = 0
         T up[3] = {zero, zero, zero}, um[3] = {zero, zero, zero};   // c_y = +1 / -1
         T* SUup = SU;                                    // interior: Up summed over z (plane z-1); x frame: Up[c_z = 0] of the virtual column, plane z
         T* SUum = SU + SUP;
-#pragma unroll
-        for (int p = 0; p < 9; ++p) {
-            const T h1 = f[2 * p + 1], h2 = f[2 * p + 2];
-            T l = zero, r = zero;
-            if (p == 0 || (p >= 3 && p <= 6)) { l = __shfl_up_sync(0xffffffffu, h1, 1); r = __shfl_down_sync(0xffffffffu, h2, 1); }
-            if (p == 0) {                                                  // +x / -x
-                if (!lane_lo) u0[1] += l;
-                if (!lane_hi) u0[1] += r;
-                ee[1] = lane_hi ? h1 : h2;
-            } else if (p == 1) { up[1] = h1; um[1] = h2; }                  // +y / -y
-            else if (p == 2) { u0[2] = h1; u0[0] = h2; }                    // +z / -z
-            else if (p == 3) {                                             // +x+y / -x-y
-                if (!lane_lo) up[1] += l;
-                if (!lane_hi) um[1] += r;
-                if (lane_hi) SUup[own_s + 1] = h1;
-                if (lane_lo) SUum[own_s - 1] = h2;
-            } else if (p == 4) {                                           // +x-y / -x+y
-                if (!lane_lo) um[1] += l;
-                if (!lane_hi) up[1] += r;
-                if (lane_hi) SUum[own_s + 1] = h1;
-                if (lane_lo) SUup[own_s - 1] = h2;
-            } else if (p == 5) {                                           // +x+z / -x-z
-                if (!lane_lo) u0[2] += l;
-                if (!lane_hi) u0[0] += r;
-                if (lane_hi) ee[2] = h1;
-                if (lane_lo) ee[0] = h2;
-            } else if (p == 6) {                                           // +x-z / -x+z
-                if (!lane_lo) u0[0] += l;
-                if (!lane_hi) u0[2] += r;
-                if (lane_hi) ee[0] = h1;
-                if (lane_lo) ee[2] = h2;
-            } else if (p == 7) { up[2] = h1; um[0] = h2; }                  // +y+z / -y-z
-            else { up[0] = h1; um[2] = h2; }                               // +y-z / -y+z
-        }
-        if (HAS_SOLID && fluid && (lk & 0x7FFFEu)) {                       // bounced-back arrivals of the next step come from this node
-            T bs = zero;
-#pragma unroll
-            for (int i = 1; i < Q; ++i)
-                if (lk >> i & 1u) bs += f[i];
-            u0[1] += bs;
-        }
+        T bs = zero;                                     // bounced-back arrivals of the next step come from this node
+        const bool do_store = fluid && store_h;
+        T* o = gk + zoff;                                // values arrive in direction order: a running pointer
+        auto put = [&](T v) {
+            if (do_store) st_global(o, v);
+            o += NP;
+            asm volatile("" : "+l"(o));                  // keep it a pointer: ptxas otherwise re-derives every address from scratch
+        };
+        collide19_pairs<T>(f, rho, omc, ux, uy, uz, ex, ey, ez,
+            [&](T h0) { put(h0); u0[1] = h0; },
+            [&](int p, T h1, T h2) {
+                put(h1);
+                put(h2);
+                if (HAS_SOLID) {
+                    if (lk >> (2 * p + 1) & 1u) bs += h1;
+                    if (lk >> (2 * p + 2) & 1u) bs += h2;
+                }
+                T l = zero, r = zero;
+                if (p == 0 || (p >= 3 && p <= 6)) { l = __shfl_up_sync(0xffffffffu, h1, 1); r = __shfl_down_sync(0xffffffffu, h2, 1); }
+                if (p == 0) {                                              // +x / -x
+                    if (!lane_lo) u0[1] += l;
+                    if (!lane_hi) u0[1] += r;
+                    ee[1] = lane_hi ? h1 : h2;
+                } else if (p == 1) { up[1] = h1; um[1] = h2; }              // +y / -y
+                else if (p == 2) { u0[2] = h1; u0[0] = h2; }                // +z / -z
+                else if (p == 3) {                                         // +x+y / -x-y
+                    up[1] += lane_lo ? zero : l;
+                    um[1] += lane_hi ? zero : r;
+                    if (lane_hi) SUup[own_s + 1] = h1;
+                    if (lane_lo) SUum[own_s - 1] = h2;
+                } else if (p == 4) {                                       // +x-y / -x+y
+                    um[1] += lane_lo ? zero : l;
+                    up[1] += lane_hi ? zero : r;
+                    if (lane_hi) SUum[own_s + 1] = h1;
+                    if (lane_lo) SUup[own_s - 1] = h2;
+                } else if (p == 5) {                                       // +x+z / -x-z
+                    if (!lane_lo) u0[2] += l;
+                    if (!lane_hi) u0[0] += r;
+                    if (lane_hi) ee[2] = h1;
+                    if (lane_lo) ee[0] = h2;
+                } else if (p == 6) {                                       // +x-z / -x+z
+                    if (!lane_lo) u0[0] += l;
+                    if (!lane_hi) u0[2] += r;
+                    if (lane_hi) ee[0] = h1;
+                    if (lane_lo) ee[2] = h2;
+                } else if (p == 7) { up[2] = h1; um[0] = h2; }              // +y+z / -y-z
+                else { up[0] = h1; um[2] = h2; }                           // +y-z / -y+z
+                // corners: only c_z = 0 directions reach a diagonal tile, so the target plane is this plane
+                if ((p == 3 || p == 4) && store_h && (lane_lo || lane_hi) && (row_lo || row_hi)) {
+                    T* cxy = ro.xy + k * ro.s_xy + zl * psxy;
+                    if (p == 3 && lane_hi && row_hi) cxy[(btyp * ntx + btxp) * 4 + 0] = h1;     // +x+y
+                    if (p == 3 && lane_lo && row_lo) cxy[(btym * ntx + btxm) * 4 + 3] = h2;     // -x-y
+                    if (p == 4 && lane_hi && row_lo) cxy[(btym * ntx + btxp) * 4 + 2] = h1;     // +x-y
+                    if (p == 4 && lane_lo && row_hi) cxy[(btyp * ntx + btxm) * 4 + 1] = h2;     // -x+y
+                }
+            });
+        if (HAS_SOLID) u0[1] += bs;
         const T p0 = acc0[0] + u0[0], pp = accp[0] + up[0], pm = accm[0] + um[0];   // complete for plane z-1
         acc0[0] = acc0[1] + u0[1]; acc0[1] = u0[2];
         accp[0] = accp[1] + up[1]; accp[1] = up[2];
@@ -506,14 +516,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         // ---- global stores that need nothing from the other warps: the y-edge and corner exports ----
         if (row_lo || row_hi) {                                            // the row beyond the tile edge receives exactly Um (Up)
             if (store_rho) (ro.y + k * ro.s_y)[zt * psy + ((row_lo ? btym : btyp) * 2 + (row_lo ? 1 : 0)) * nx + x] = row_lo ? pm : pp;
-            // corners: only c_z = 0 directions reach a diagonal tile, so the target plane is this plane
-            if (store_h && (lane_lo || lane_hi)) {
-                T* cxy = ro.xy + k * ro.s_xy + zl * psxy;
-                if (lane_hi && row_hi) cxy[(btyp * ntx + btxp) * 4 + 0] = f[7];     // +x+y
-                if (lane_lo && row_lo) cxy[(btym * ntx + btxm) * 4 + 3] = f[8];     // -x-y
-                if (lane_hi && row_lo) cxy[(btym * ntx + btxp) * 4 + 2] = f[9];     // +x-y
-                if (lane_lo && row_hi) cxy[(btyp * ntx + btxm) * 4 + 1] = f[10];    // -x+y
-            }
         }
 
         TRACE(t == 0, it, 5);
