@@ -283,6 +283,21 @@ def test_headline_512_cube_sampled_moments_and_invariants(oracle_mod):
         assert np.abs(p1 - p0).max() < 1e-7                       # total momentum (|P| ~ 0, N = 1.3e8)
 
 
+def test_tma_kernel_with_32x4_tiles():
+    """LB_TMA_TY=4 selects the 32 x 4 tile / two CTAs per SM variant of the TMA kernel when the library creates a
+    context: the small-box, tile-edge and solid parity cases are run again under it in a child process."""
+    import os
+    import subprocess
+    import sys
+    if os.environ.get("LB_TMA_TY") == "4":
+        pytest.skip("already inside the child run")
+    env = dict(os.environ, LB_TMA_TY="4")
+    sel = "tma and (random_populations or ragged or spheres_64 or wall_and_single)"
+    r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-m", "gpu", "-x", "-q", "-k", sel],
+                       env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+
+
 # ---------------------------------------------------------------------------------------------
 # API behaviour on the device
 # ---------------------------------------------------------------------------------------------
