@@ -25,8 +25,10 @@
  *   Values     the ABI speaks double for both LB_F64 and LB_F32 contexts; an LB_F32 context
  *              rounds to float on the way in and widens on the way out.
  *   Errors     lb_create* return NULL on failure; all other calls return LB_OK or a negative
- *              code; lb_last_error() holds a message for the calling thread.  No exception
- *              crosses the boundary.
+ *              code; lb_last_error() holds a message and lb_last_error_code() the code of the
+ *              last failure on the calling thread.  No exception crosses the boundary.
+ *   Device     a context lives on the CUDA device that is current when it is created; every
+ *              later call switches to that device for its own duration.
  *   Ordering   lb_step only enqueues work on the context's stream and may return before the
  *              GPU finishes; every getter synchronises that stream.
  *   Threads    one context may be used from one thread at a time.
@@ -43,6 +45,7 @@ typedef struct lb_ctx lb_ctx;          /* opaque; owned by the library */
 enum { LB_OK = 0, LB_EINVAL = -1, LB_ENOMEM = -2, LB_ECUDA = -3, LB_ESTATE = -4 };
 enum { LB_F64 = 0, LB_F32 = 1 };
 enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2, LB_KERNEL_TMA = 3 };
+enum { LB_OPT_ZC = 1 };                /* options of lb_set_option */
 
 /* Create a context for an nx*ny*nz periodic box holding two fluids with BGK
  * relaxation times tau_r, tau_b (Eq. 1; omega_k = 1/tau_k) coupled by the
@@ -51,8 +54,10 @@ enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2, LB_KERN
  * fp64 populations, the library's own stream.
  * NULL (LB_EINVAL) if a dimension is < 1, tau <= 0.5 or not finite (Eq. 2, PAPER.md:84-86,
  * needs 0 < omega < 2), or G is not finite; NULL (LB_ENOMEM / LB_ECUDA) if device memory or
- * the device is not available.  Device memory: 2 population buffers of 38*N values plus
- * about 17 bytes per node. */
+ * the device is not available; lb_last_error_code() tells which.  Device memory: 2 population
+ * buffers of 38*N values; the carried density, 2 x 2 arrays of N values plus tile-edge arrays
+ * (about 54 bytes per node in fp64, 27 in fp32, when nx % 32 == 0 and ny % 8 == 0; 32 / 16
+ * otherwise); 4 bytes per node of link words; a staging buffer of 40 bytes x min(N, 2^22). */
 lb_ctx* lb_create(int nx, int ny, int nz, double tau_r, double tau_b, double G);
 
 /* Same, with the population type (LB_F64 / LB_F32: "fp32 populations and fields", all
@@ -115,11 +120,20 @@ int lb_get_diagnostics(lb_ctx* ctx, double mass[2], double momentum[3]);
  * reads and writes every population once per step, populations pulled with per-thread loads;
  * LB_KERNEL_TMA = the same single pass with the populations staged in shared memory by the TMA
  * unit (the fastest; needs nx % 32 == 0 and ny % 8 == 0 like ONEPASS); LB_KERNEL_AUTO (default) =
- * TMA when the box shape allows it, else TWOPASS.  LB_EINVAL if the box shape does not allow `kind`. */
+ * TMA when the box shape allows it (ONEPASS if the driver cannot encode the tensor maps), else
+ * TWOPASS: boxes whose sides are not multiples of the 32 x 8 tile run about 1.5 x slower.
+ * LB_EINVAL if the box shape does not allow `kind`. */
 int lb_set_kernel(lb_ctx* ctx, int kind);
 
 /* The kernel lb_step will use (LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS or LB_KERNEL_TMA; never AUTO); -1 for a NULL context. */
 int lb_get_kernel(const lb_ctx* ctx);
+
+/* Tuning and modes.  LB_OPT_ZC: planes per CTA of the one-pass kernels (each CTA marches over
+ * value z planes and re-collides one more at either end); 0 = the library's heuristic (default).
+ * LB_EINVAL for an unknown option or a value out of range.  lb_get_option returns the value in
+ * effect (for LB_OPT_ZC: the planes per CTA the current kernel will use), -1 on error. */
+int lb_set_option(lb_ctx* ctx, int option, long long value);
+long long lb_get_option(const lb_ctx* ctx, int option);
 
 /* Number of kernel launches this context has enqueued so far (for bench.py's gpu_launches). */
 long long lb_launch_count(const lb_ctx* ctx);
@@ -129,6 +143,10 @@ int lb_sync(lb_ctx* ctx);
 
 /* Message for the last failure on the calling thread ("" if none). */
 const char* lb_last_error(void);
+
+/* Code of the last failure on the calling thread (LB_OK if none): tells LB_EINVAL, LB_ENOMEM
+ * and LB_ECUDA apart after lb_create* returned NULL. */
+int lb_last_error_code(void);
 
 /* Library version string. */
 const char* lb_version(void);

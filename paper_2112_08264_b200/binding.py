@@ -17,6 +17,7 @@ import numpy as np
 LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 LB_F64, LB_F32 = 0, 1
 LB_KERNEL_AUTO, LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA = 0, 1, 2, 3
+LB_OPT_ZC = 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "_lib", "liblb_b200.so")
@@ -26,7 +27,7 @@ SYMBOLS = (
     "lb_create", "lb_create_ex", "lb_destroy", "lb_set_fields", "lb_set_solid_mask",
     "lb_set_populations", "lb_step", "lb_get_populations", "lb_get_moments",
     "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
-    "lb_sync", "lb_last_error", "lb_version",
+    "lb_set_option", "lb_get_option", "lb_sync", "lb_last_error", "lb_last_error_code", "lb_version",
 )
 
 _dp = C.POINTER(C.c_double)
@@ -67,6 +68,9 @@ def lib() -> C.CDLL:
     L.lb_launch_count.restype = C.c_longlong
     L.lb_launch_count.argtypes = [C.c_void_p]
     L.lb_get_kernel.argtypes = [C.c_void_p]
+    L.lb_set_option.argtypes = [C.c_void_p, C.c_int, C.c_longlong]
+    L.lb_get_option.restype = C.c_longlong
+    L.lb_get_option.argtypes = [C.c_void_p, C.c_int]
     L.lb_sync.argtypes = [C.c_void_p]
     L.lb_last_error.restype = C.c_char_p
     L.lb_version.restype = C.c_char_p
@@ -101,17 +105,21 @@ def _host_f64(a, n, name):
     return a
 
 
+def lb_last_error_code() -> int:
+    return int(lib().lb_last_error_code())
+
+
 def lb_create(nx, ny, nz, tau_r, tau_b, G):
     h = lib().lb_create(nx, ny, nz, tau_r, tau_b, G)
     if not h:
-        raise LBError(LB_EINVAL, lb_last_error())
+        raise LBError(lb_last_error_code(), lb_last_error())
     return h
 
 
 def lb_create_ex(nx, ny, nz, tau_r, tau_b, G, dtype=LB_F64, cuda_stream=None):
     h = lib().lb_create_ex(nx, ny, nz, tau_r, tau_b, G, dtype, cuda_stream)
     if not h:
-        raise LBError(LB_EINVAL, lb_last_error())
+        raise LBError(lb_last_error_code(), lb_last_error())
     return h
 
 
@@ -174,6 +182,14 @@ def lb_kernel_name(h) -> str:
     return KERNEL_NAMES.get(int(lib().lb_get_kernel(h)), "?")
 
 
+def lb_set_option(h, option, value):
+    _chk(lib().lb_set_option(h, option, value))
+
+
+def lb_get_option(h, option) -> int:
+    return int(lib().lb_get_option(h, option))
+
+
 def lb_launch_count(h) -> int:
     return int(lib().lb_launch_count(h))
 
@@ -230,6 +246,12 @@ class Box:
 
     def set_kernel(self, kind):
         lb_set_kernel(self.h, kind)
+
+    def set_option(self, option, value):
+        lb_set_option(self.h, option, value)
+
+    def get_option(self, option):
+        return lb_get_option(self.h, option)
 
     def launch_count(self):
         return lb_launch_count(self.h)

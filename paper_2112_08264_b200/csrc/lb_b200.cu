@@ -33,6 +33,7 @@ struct lb_ctx {
     long long NP;      // plane stride in elements: N rounded up so every [k][i] plane is 256-B aligned
     int dtype;
     double tau[2], G;
+    int device;        // CUDA device the context lives on (the current device at lb_create*)
     cudaStream_t stream;
     bool own_stream;
     void* f[2];        // ping-pong population buffers, [k][i][NP]; f[cur] = h-state, f[cur^1] = scratch
@@ -50,10 +51,11 @@ struct lb_ctx {
     int kernel_req;
     int zc;            // planes per CTA of the one-pass kernel
     int zc_tma;        // ... of the TMA kernel
-    int tma_ty;        // tile height of the TMA kernel: 8 (one CTA per SM) or 4 (two)
-    CUtensorMap tmap[2][3];   // [buffer][narrow box 32 x TY, wide box (32 + 16 B) x TY, wrapped-column box 16 B x TY] over [k*19+i][z][y][x]
+    CUtensorMap tmap[2][3];   // [buffer][narrow box 32 x 8, wide box (32 + 16 B) x 8, wrapped-column box 16 B x 8; each 2 planes deep] over [plane][z][y][x]
     bool have_tmap;
-    double* stage;     // device staging, STAGE_NODES * 5 doubles
+    double* stage;     // device staging, stage_nodes * 5 doubles
+    long long stage_nodes;   // min(N, STAGE_NODES)
+    int zc_req;        // lb_set_option(LB_OPT_ZC): planes per CTA of the one-pass kernels, 0 = heuristic
     double* diag_part; // [DIAG_BLOCKS][5]
     double* diag_out;  // [5]
     long long launches;
@@ -67,12 +69,24 @@ constexpr unsigned SOLID_BIT = 1u << 31;
 constexpr int OP_TX = 32, OP_TY = 8;
 
 thread_local std::string g_err;
+thread_local int g_err_code = LB_OK;
 
-int fail(int code, const char* what) { g_err = what; return code; }
+int fail(int code, const char* what) { g_err = what; g_err_code = code; return code; }
 int fail_cuda(cudaError_t e, const char* where) {
     g_err = std::string(where) + ": " + cudaGetErrorString(e);
-    return LB_ECUDA;
+    g_err_code = e == cudaErrorMemoryAllocation ? LB_ENOMEM : LB_ECUDA;
+    return g_err_code;
 }
+
+// every ABI call runs on the context's device, whatever the caller's current device is
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != dev) cudaSetDevice(dev); else prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 #define CU(call)                                                         \
     do {                                                                 \
         cudaError_t e__ = (call);                                        \
@@ -81,8 +95,8 @@ int fail_cuda(cudaError_t e, const char* where) {
 
 size_t esize(const lb_ctx* c) { return c->dtype == LB_F64 ? 8 : 4; }
 
-template <typename T> __device__ __forceinline__ T* plane(T* f, long long NP, int k, int i) { return f + (long long)(k * Q + i) * NP; }
-template <typename T> __device__ __forceinline__ const T* plane(const T* f, long long NP, int k, int i) { return f + (long long)(k * Q + i) * NP; }
+template <typename T> __device__ __forceinline__ T* plane(T* f, long long NP, int k, int i) { return f + (long long)pop_plane(k, i) * NP; }
+template <typename T> __device__ __forceinline__ const T* plane(const T* f, long long NP, int k, int i) { return f + (long long)pop_plane(k, i) * NP; }
 
 // periodic neighbour offsets of node n, any box shape
 struct Nbr {
@@ -460,9 +474,9 @@ int stream_to_scratch(lb_ctx* c) {
 constexpr int OP_RESIDENT_CTAS = 148 * 2;
 
 // planes per CTA: every chunk re-collides 2 extra planes, so long chunks; but the grid should
-// still be several waves of the resident CTAs.  LB_ONEPASS_ZC overrides (tuning).
+// still be several waves of the resident CTAs.  lb_set_option(LB_OPT_ZC) overrides.
 int onepass_zc(const lb_ctx* c) {
-    if (const char* e = std::getenv("LB_ONEPASS_ZC")) { const int v = std::atoi(e); if (v >= 1) return v < c->nz ? v : c->nz; }
+    if (c->zc_req >= 1) return c->zc_req < c->nz ? c->zc_req : c->nz;
     const long long tiles = (long long)(c->nx / OP_TX) * (c->ny / OP_TY);
     const long long chunks_wanted = (OP_RESIDENT_CTAS * 4 + tiles - 1) / (tiles > 0 ? tiles : 1);
     long long zc = c->nz / (chunks_wanted > 0 ? chunks_wanted : 1);
@@ -488,11 +502,6 @@ template <typename T, bool HAS_SOLID>
 int launch_onepass(lb_ctx* c) {
     auto kern = k_step_pull<T, HAS_SOLID, OP_TX, OP_TY>;
     constexpr size_t smem = onepass_smem_bytes<T, OP_TX, OP_TY>();
-    static bool configured = false;                         // per instantiation
-    if (!configured) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
-        configured = true;
-    }
     const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc - 1) / c->zc);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
     kern<<<grid, OP_TX * OP_TY, smem, c->stream>>>(static_cast<const T*>(c->f[c->cur]), static_cast<T*>(c->f[c->cur ^ 1]),
@@ -537,7 +546,7 @@ bool make_tmaps(lb_ctx* c) {
     for (int b = 0; b < 2; ++b)
         for (int w = 0; w < 3; ++w) {
             const cuuint32_t pad = cuuint32_t(16 / int(es));
-            const cuuint32_t box[4] = {w == 0 ? cuuint32_t(OP_TX) : (w == 1 ? OP_TX + pad : pad), cuuint32_t(c->tma_ty), 1, 1};
+            const cuuint32_t box[4] = {w == 0 ? cuuint32_t(OP_TX) : (w == 1 ? OP_TX + pad : pad), cuuint32_t(OP_TY), 1, 2};   // both components (pop_plane)
             if (enc(&c->tmap[b][w], dt, 4, c->f[b], gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
                 return false;
@@ -545,21 +554,16 @@ bool make_tmaps(lb_ctx* c) {
     return true;
 }
 
-template <typename T, bool HAS_SOLID, int TY>
+template <typename T, bool HAS_SOLID>
 int launch_tma(lb_ctx* c) {
-    auto kern = k_step_tma<T, HAS_SOLID, TY>;
-    constexpr size_t smem = TmaLayout<T, TY>::BYTES;
-    static bool configured = false;                         // per instantiation
-    if (!configured) {
-        CU(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)));
-        configured = true;
-    }
-    const dim3 grid(c->nx / OP_TX, c->ny / TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
+    auto kern = k_step_tma<T, HAS_SOLID, OP_TY>;
+    constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
+    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    kern<<<grid, 2 * OP_TX * TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
-                                                        static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
-                                                        rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
-                                                        c->zc_tma, om_r, om_b, G);
+    kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
+                                                           static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
+                                                           rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
+                                                           c->zc_tma, om_r, om_b, G);
     c->launches += 1;
     CU(cudaGetLastError());
     return LB_OK;
@@ -569,22 +573,35 @@ template <typename T>
 int step_tma(lb_ctx* c) {
     int rc = ensure_rho<T>(c);
     if (rc != LB_OK) return rc;
-    if (c->tma_ty == 4) rc = c->has_solid ? launch_tma<T, true, 4>(c) : launch_tma<T, false, 4>(c);
-    else rc = c->has_solid ? launch_tma<T, true, 8>(c) : launch_tma<T, false, 8>(c);
+    rc = c->has_solid ? launch_tma<T, true>(c) : launch_tma<T, false>(c);
     if (rc != LB_OK) return rc;
     c->cur ^= 1;
     c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
     return LB_OK;
 }
 
+// The one-pass kernels use more dynamic shared memory than the default limit: opt in once per context (the attribute is
+// per device and per function; setting it again is harmless).
+template <typename T>
+int configure_onepass_kernels() {
+    CU(cudaFuncSetAttribute(k_step_pull<T, false, OP_TX, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(onepass_smem_bytes<T, OP_TX, OP_TY>())));
+    CU(cudaFuncSetAttribute(k_step_pull<T, true, OP_TX, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(onepass_smem_bytes<T, OP_TX, OP_TY>())));
+    CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
+    CU(cudaFuncSetAttribute(k_step_tma<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
+    return LB_OK;
+}
+
 // planes per CTA of the TMA kernel: every chunk re-collides 2 extra planes (long chunks), but the grid should fill the
 // SMs (one CTA each) in whole waves, and more waves balance better.  Measured on B200: 256^3 -> 64, 512^3 -> 256.
 int tma_zc(const lb_ctx* c) {
-    if (const char* e = std::getenv("LB_ONEPASS_ZC")) { const int v = std::atoi(e); if (v >= 1) return v < c->nz ? v : c->nz; }
-    int dev = 0, sms = 148;
-    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const double tiles = double(c->nx / OP_TX) * (c->ny / c->tma_ty);
-    if (c->tma_ty == 4) sms *= 2;
+    if (c->zc_req >= 1) {                                             // the kernel wants whole chunks: the largest divisor of nz <= the request
+        int zc = c->zc_req < c->nz ? c->zc_req : c->nz;
+        while (c->nz % zc != 0) --zc;
+        return zc;
+    }
+    int sms = 148;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
+    const double tiles = double(c->nx / OP_TX) * (c->ny / OP_TY);
     int best = c->nz;
     double best_cost = 1e300;
     for (int zc = 1; zc <= c->nz; ++zc) {
@@ -619,10 +636,12 @@ int lb_debug_trace(long long* out) { return cudaMemcpyFromSymbol(out, lb::g_trac
 #endif
 
 const char* lb_last_error(void) { return g_err.c_str(); }
+int lb_last_error_code(void) { return g_err_code; }
 const char* lb_version(void) { return "lb-b200 0.2 (sm_100a)"; }
 
 lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double G, int dtype, void* cuda_stream) {
     g_err.clear();
+    g_err_code = LB_OK;
     if (nx < 1 || ny < 1 || nz < 1) { fail(LB_EINVAL, "box dimensions must be >= 1"); return nullptr; }
     if ((long long)nx * ny * nz > (1ll << 31) - 1) { fail(LB_EINVAL, "box too large (N must fit in 31 bits)"); return nullptr; }
     if (!(tau_r > 0.5) || !(tau_b > 0.5) || !std::isfinite(tau_r) || !std::isfinite(tau_b)) {
@@ -639,6 +658,8 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     lb_ctx* c = new (std::nothrow) lb_ctx();
     if (!c) { fail(LB_ENOMEM, "host allocation failed"); return nullptr; }
     std::memset(c, 0, sizeof(*c));
+    e = cudaGetDevice(&c->device);
+    if (e != cudaSuccess) { fail_cuda(e, "cudaGetDevice"); delete c; return nullptr; }
     c->nx = nx; c->ny = ny; c->nz = nz;
     c->N = (long long)nx * ny * nz;
     c->NP = round64(c->N);
@@ -657,8 +678,8 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     ok = ok && cudaMalloc(&c->f[1], fbytes) == cudaSuccess;
     for (int r = 0; r < 2; ++r) ok = ok && cudaMalloc(&c->rho_in[r], size_t(2) * c->NP * es) == cudaSuccess;
     if (onepass_ok(c)) {
-        const long long ntx = nx / OP_TX, nty = ny / 4;    // sized for the smallest tile height any kernel uses
-        c->s_x = round64((long long)nz * nty * ntx * 2 * 4);
+        const long long ntx = nx / OP_TX, nty = ny / OP_TY;
+        c->s_x = round64((long long)nz * nty * ntx * 2 * OP_TY);
         c->s_y = round64((long long)nz * nty * 2 * nx);
         c->s_xy = round64((long long)nz * nty * ntx * 4);
         for (int r = 0; r < 2; ++r) {
@@ -668,7 +689,8 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
         }
     }
     ok = ok && cudaMalloc(&c->links, size_t(c->N) * sizeof(unsigned)) == cudaSuccess;
-    ok = ok && cudaMalloc(&c->stage, size_t(STAGE_NODES) * 5 * sizeof(double)) == cudaSuccess;
+    c->stage_nodes = c->N < STAGE_NODES ? c->N : STAGE_NODES;
+    ok = ok && cudaMalloc(&c->stage, size_t(c->stage_nodes) * 5 * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->diag_part, size_t(DIAG_BLOCKS) * 5 * sizeof(double)) == cudaSuccess;
     ok = ok && cudaMalloc(&c->diag_out, 5 * sizeof(double)) == cudaSuccess;
     if (ok) {
@@ -678,12 +700,14 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     }
     if (!ok) {
         e = cudaGetLastError();
-        g_err = std::string("device allocation failed: ") + cudaGetErrorString(e);
         lb_destroy(c);
-        return nullptr;                                  // LB_ENOMEM
+        fail_cuda(e, "device allocation failed");        // LB_ENOMEM for an out-of-memory, LB_ECUDA otherwise
+        return nullptr;
     }
-    c->tma_ty = 8;
-    if (const char* e = std::getenv("LB_TMA_TY")) { if (std::atoi(e) == 4) c->tma_ty = 4; }
+    if (onepass_ok(c) && (dtype == LB_F64 ? configure_onepass_kernels<double>() : configure_onepass_kernels<float>()) != LB_OK) {
+        lb_destroy(c);
+        return nullptr;                                  // LB_ECUDA, message set
+    }
     c->have_tmap = onepass_ok(c) && make_tmaps(c);
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
@@ -698,6 +722,7 @@ lb_ctx* lb_create(int nx, int ny, int nz, double tau_r, double tau_b, double G) 
 
 void lb_destroy(lb_ctx* c) {
     if (!c) return;
+    DeviceGuard guard(c->device);
     cudaStreamSynchronize(c->stream);
     cudaFree(c->f[0]); cudaFree(c->f[1]); cudaFree(c->links);
     for (int r = 0; r < 2; ++r) { cudaFree(c->rho_in[r]); cudaFree(c->rho_x[r]); cudaFree(c->rho_y[r]); cudaFree(c->rho_xy[r]); }
@@ -708,6 +733,7 @@ void lb_destroy(lb_ctx* c) {
 
 int lb_sync(lb_ctx* c) {
     if (!c) return fail(LB_EINVAL, "NULL context");
+    DeviceGuard guard(c->device);
     CU(cudaStreamSynchronize(c->stream));
     return LB_OK;
 }
@@ -715,6 +741,29 @@ int lb_sync(lb_ctx* c) {
 long long lb_launch_count(const lb_ctx* c) { return c ? c->launches : 0; }
 
 int lb_get_kernel(const lb_ctx* c) { return c ? c->kernel : -1; }
+
+int lb_set_option(lb_ctx* c, int option, long long value) {
+    if (!c) return fail(LB_EINVAL, "NULL context");
+    DeviceGuard guard(c->device);
+    switch (option) {
+    case LB_OPT_ZC:
+        if (value < 0 || value > c->nz) return fail(LB_EINVAL, "LB_OPT_ZC: 0 (heuristic) or 1..nz planes per CTA");
+        c->zc_req = int(value);
+        c->zc = onepass_zc(c);
+        c->zc_tma = tma_zc(c);
+        return LB_OK;
+    default:
+        return fail(LB_EINVAL, "unknown option");
+    }
+}
+
+long long lb_get_option(const lb_ctx* c, int option) {
+    if (!c) return -1;
+    switch (option) {
+    case LB_OPT_ZC: return c->kernel == LB_KERNEL_TMA ? c->zc_tma : c->zc;
+    default: return -1;
+    }
+}
 
 int lb_set_kernel(lb_ctx* c, int kind) {
     if (!c) return fail(LB_EINVAL, "NULL context");
@@ -729,6 +778,7 @@ int lb_set_kernel(lb_ctx* c, int kind) {
 
 int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
     if (!c || !mask) return fail(LB_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const bool f64 = c->dtype == LB_F64;
     int rc;
     // the fields already set are defined on nodes (f): take them out of the h-state under the OLD links
@@ -736,8 +786,12 @@ int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
         rc = f64 ? stream_to_scratch<double>(c) : stream_to_scratch<float>(c);
         if (rc != LB_OK) return rc;
     }
-    unsigned char* d_mask = nullptr;
-    CU(cudaMalloc(&d_mask, size_t(c->N)));
+    bool any_solid = false;
+    for (long long n = 0; n < c->N && !any_solid; ++n) any_solid = mask[n] != 0;
+    // the mask travels through the staging buffer when it fits there, else through a temporary
+    const bool own_tmp = size_t(c->N) > size_t(c->stage_nodes) * 5 * sizeof(double);
+    unsigned char* d_mask = reinterpret_cast<unsigned char*>(c->stage);
+    if (own_tmp) CU(cudaMalloc(&d_mask, size_t(c->N)));
     cudaError_t e = cudaMemcpyAsync(d_mask, mask, size_t(c->N), cudaMemcpyHostToDevice, c->stream);
     if (e == cudaSuccess) {
         k_build_links<<<blocks_for(c->N, 256), 256, 0, c->stream>>>(d_mask, c->links, c->nx, c->ny, c->nz);
@@ -745,10 +799,14 @@ int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
-    cudaFree(d_mask);
+    if (own_tmp) cudaFree(d_mask);
     if (e != cudaSuccess) return fail_cuda(e, "lb_set_solid_mask");
-    c->has_solid = true;   // a mask of all zeros still takes the (slower) link-checking kernels
+    c->has_solid = any_solid;   // a mask without solid nodes keeps the plain (no link word) kernels
     c->rho_valid = false;
+    if (!any_solid) {
+        if (c->have_fields) return c->dtype == LB_F64 ? unstream_scratch<double>(c) : unstream_scratch<float>(c);
+        return LB_OK;
+    }
     // S8: solid nodes hold exactly 0 in both buffers (the step kernels never write them)
     rc = f64 ? zero_solids<double>(c, c->cur ^ 1) : zero_solids<float>(c, c->cur ^ 1);
     if (rc != LB_OK) return rc;
@@ -758,15 +816,16 @@ int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
 
 int lb_set_fields(lb_ctx* c, const double* rho_r, const double* rho_b, const double* ux, const double* uy, const double* uz) {
     if (!c || !rho_r || !rho_b) return fail(LB_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const int nu = (ux != nullptr) + (uy != nullptr) + (uz != nullptr);
     if (nu != 0 && nu != 3) return fail(LB_EINVAL, "ux, uy, uz must be all NULL or all non-NULL");
     const double* src[5] = {rho_r, rho_b, ux, uy, uz};
     void* scratch = c->f[c->cur ^ 1];
-    for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES) {
-        const long long cnt = (c->N - n0 < STAGE_NODES) ? c->N - n0 : STAGE_NODES;
+    for (long long n0 = 0; n0 < c->N; n0 += c->stage_nodes) {
+        const long long cnt = (c->N - n0 < c->stage_nodes) ? c->N - n0 : c->stage_nodes;
         double* st[5];
         for (int a = 0; a < 5; ++a) {
-            st[a] = src[a] ? c->stage + a * STAGE_NODES : nullptr;
+            st[a] = src[a] ? c->stage + a * c->stage_nodes : nullptr;
             if (src[a]) CU(cudaMemcpyAsync(st[a], src[a] + n0, size_t(cnt) * sizeof(double), cudaMemcpyHostToDevice, c->stream));
         }
         const unsigned* lk = c->has_solid ? c->links : nullptr;
@@ -786,15 +845,17 @@ int lb_set_fields(lb_ctx* c, const double* rho_r, const double* rho_b, const dou
 
 int lb_set_populations(lb_ctx* c, const double* f) {
     if (!c || !f) return fail(LB_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     void* scratch = c->f[c->cur ^ 1];
-    for (int q = 0; q < NPOP; ++q) {
+    for (int q = 0; q < NPOP; ++q) {                    // ABI order [k][i] -> plane pop_plane(k, i)
         const double* src = f + (long long)q * c->N;
+        const long long pq = pop_plane(q / Q, q % Q);
         if (c->dtype == LB_F64) {
-            CU(cudaMemcpyAsync(static_cast<double*>(scratch) + (long long)q * c->NP, src, size_t(c->N) * 8, cudaMemcpyHostToDevice, c->stream));
+            CU(cudaMemcpyAsync(static_cast<double*>(scratch) + pq * c->NP, src, size_t(c->N) * 8, cudaMemcpyHostToDevice, c->stream));
         } else {
-            float* dst = static_cast<float*>(scratch) + (long long)q * c->NP;
-            for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES * 5) {
-                const long long cnt = (c->N - n0 < STAGE_NODES * 5) ? c->N - n0 : STAGE_NODES * 5;
+            float* dst = static_cast<float*>(scratch) + pq * c->NP;
+            for (long long n0 = 0; n0 < c->N; n0 += c->stage_nodes * 5) {
+                const long long cnt = (c->N - n0 < c->stage_nodes * 5) ? c->N - n0 : c->stage_nodes * 5;
                 CU(cudaMemcpyAsync(c->stage, src + n0, size_t(cnt) * 8, cudaMemcpyHostToDevice, c->stream));
                 k_from_double<float><<<blocks_for(cnt, 256), 256, 0, c->stream>>>(c->stage, dst + n0, cnt);
                 c->launches++;
@@ -816,6 +877,7 @@ int lb_set_populations(lb_ctx* c, const double* f) {
 
 int lb_step(lb_ctx* c, int nsteps) {
     if (!c) return fail(LB_EINVAL, "NULL context");
+    DeviceGuard guard(c->device);
     if (nsteps < 0) return fail(LB_EINVAL, "nsteps must be >= 0");
     if (!c->have_fields) return fail(LB_ESTATE, "lb_step before lb_set_fields / lb_set_populations");
     for (int s = 0; s < nsteps; ++s) {
@@ -830,17 +892,19 @@ int lb_step(lb_ctx* c, int nsteps) {
 
 int lb_get_populations(lb_ctx* c, double* f) {
     if (!c || !f) return fail(LB_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const int rc = c->dtype == LB_F64 ? stream_to_scratch<double>(c) : stream_to_scratch<float>(c);
     if (rc != LB_OK) return rc;
     const void* scratch = c->f[c->cur ^ 1];
-    for (int q = 0; q < NPOP; ++q) {
+    for (int q = 0; q < NPOP; ++q) {                    // plane pop_plane(k, i) -> ABI order [k][i]
         double* dst = f + (long long)q * c->N;
+        const long long pq = pop_plane(q / Q, q % Q);
         if (c->dtype == LB_F64) {
-            CU(cudaMemcpyAsync(dst, static_cast<const double*>(scratch) + (long long)q * c->NP, size_t(c->N) * 8, cudaMemcpyDeviceToHost, c->stream));
+            CU(cudaMemcpyAsync(dst, static_cast<const double*>(scratch) + pq * c->NP, size_t(c->N) * 8, cudaMemcpyDeviceToHost, c->stream));
         } else {
-            const float* src = static_cast<const float*>(scratch) + (long long)q * c->NP;
-            for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES * 5) {
-                const long long cnt = (c->N - n0 < STAGE_NODES * 5) ? c->N - n0 : STAGE_NODES * 5;
+            const float* src = static_cast<const float*>(scratch) + pq * c->NP;
+            for (long long n0 = 0; n0 < c->N; n0 += c->stage_nodes * 5) {
+                const long long cnt = (c->N - n0 < c->stage_nodes * 5) ? c->N - n0 : c->stage_nodes * 5;
                 k_to_double<float><<<blocks_for(cnt, 256), 256, 0, c->stream>>>(src + n0, c->stage, cnt);
                 c->launches++;
                 CU(cudaGetLastError());
@@ -854,12 +918,13 @@ int lb_get_populations(lb_ctx* c, double* f) {
 
 int lb_get_moments(lb_ctx* c, double* rho_r, double* rho_b, double* ux, double* uy, double* uz) {
     if (!c) return fail(LB_EINVAL, "NULL context");
+    DeviceGuard guard(c->device);
     double* dst[5] = {rho_r, rho_b, ux, uy, uz};
     const unsigned* lk = c->has_solid ? c->links : nullptr;
-    for (long long n0 = 0; n0 < c->N; n0 += STAGE_NODES) {
-        const long long cnt = (c->N - n0 < STAGE_NODES) ? c->N - n0 : STAGE_NODES;
+    for (long long n0 = 0; n0 < c->N; n0 += c->stage_nodes) {
+        const long long cnt = (c->N - n0 < c->stage_nodes) ? c->N - n0 : c->stage_nodes;
         double* st[5];
-        for (int a = 0; a < 5; ++a) st[a] = c->stage + a * STAGE_NODES;
+        for (int a = 0; a < 5; ++a) st[a] = c->stage + a * c->stage_nodes;
         if (c->dtype == LB_F64)
             k_moments_out<double><<<blocks_for(cnt, 128), 128, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, n0, cnt, st[0], st[1], st[2], st[3], st[4]);
         else
@@ -875,8 +940,9 @@ int lb_get_moments(lb_ctx* c, double* rho_r, double* rho_b, double* ux, double* 
 
 int lb_get_link_mask(lb_ctx* c, unsigned int* links) {
     if (!c || !links) return fail(LB_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     unsigned* st = reinterpret_cast<unsigned*>(c->stage);
-    const long long chunk = STAGE_NODES * 10;          // staging holds 5*STAGE_NODES doubles
+    const long long chunk = c->stage_nodes * 10;          // staging holds 5*c->stage_nodes doubles
     for (long long n0 = 0; n0 < c->N; n0 += chunk) {
         const long long cnt = (c->N - n0 < chunk) ? c->N - n0 : chunk;
         k_links_out<<<blocks_for(cnt, 256), 256, 0, c->stream>>>(c->links + n0, st, cnt);
@@ -890,6 +956,7 @@ int lb_get_link_mask(lb_ctx* c, unsigned int* links) {
 
 int lb_get_diagnostics(lb_ctx* c, double mass[2], double momentum[3]) {
     if (!c || !mass || !momentum) return fail(LB_EINVAL, "NULL argument");
+    DeviceGuard guard(c->device);
     const unsigned* lk = c->has_solid ? c->links : nullptr;
     if (c->dtype == LB_F64)
         k_diag_partial<double><<<DIAG_BLOCKS, 256, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, c->diag_part);

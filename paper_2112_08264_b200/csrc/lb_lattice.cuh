@@ -11,6 +11,11 @@ namespace lb {
 constexpr int Q = 19;
 constexpr int NPOP = 2 * Q;          // two components
 
+// Plane of population (component k, direction i) inside a population buffer [NPOP][NP]: direction-major, the two
+// components of a direction adjacent, so that one TMA box (x, y, z, 2 planes) brings both (lb_tma.cuh).  Private to
+// the library: the ABI's order [k][i] is produced by the transfer calls.
+__host__ __device__ constexpr int pop_plane(int k, int i) { return 2 * i + k; }
+
 // c_i of the ODD member of pair p (direction 2p+1); the even member is its negative.
 __host__ __device__ constexpr int pair_cx(int p) { return (p == 0 || p == 3 || p == 4 || p == 5 || p == 6) ? 1 : 0; }
 __host__ __device__ constexpr int pair_cy(int p) { return (p == 1 || p == 3 || p == 7 || p == 8) ? 1 : (p == 4 ? -1 : 0); }
@@ -70,30 +75,6 @@ __device__ __forceinline__ void collide19(T (&f)[Q], T rho, T omc, T ux, T uy, T
         const T asym = (T(3) * wr) * (ce - omc * cu);
         f[2 * p + 1] = omc * f[2 * p + 1] + (sym + asym);
         f[2 * p + 2] = omc * f[2 * p + 2] + (sym - asym);
-    }
-}
-
-// The same collision, handing every post-collision value to `emit(i, value)` as soon as it exists, so that the caller's
-// stores interleave with the arithmetic instead of queueing up behind it.
-template <typename T, typename Emit>
-__device__ __forceinline__ void collide19_emit(T (&f)[Q], T rho, T omc, T ux, T uy, T uz, T ex, T ey, T ez, Emit emit) {
-    const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
-    const T ae = T(1) - T(1.5) * (ex * ex + ey * ey + ez * ez);
-    f[0] = omc * f[0] + w_rest<T>() * rho * (ae - omc * a0);
-    emit(0, f[0]);
-#pragma unroll
-    for (int p = 0; p < 9; ++p) {
-        const T cu = cdot<T>(p, ux, uy, uz);
-        const T ce = cdot<T>(p, ex, ey, ez);
-        const T wr = w_pair<T>(p) * rho;
-        const T s0 = a0 + T(4.5) * cu * cu;
-        const T se = ae + T(4.5) * ce * ce;
-        const T sym = wr * (se - omc * s0);
-        const T asym = (T(3) * wr) * (ce - omc * cu);
-        f[2 * p + 1] = omc * f[2 * p + 1] + (sym + asym);
-        f[2 * p + 2] = omc * f[2 * p + 2] + (sym - asym);
-        emit(2 * p + 1, f[2 * p + 1]);
-        emit(2 * p + 2, f[2 * p + 2]);
     }
 }
 

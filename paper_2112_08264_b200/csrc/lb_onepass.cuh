@@ -203,9 +203,8 @@ k_step_pull(const T* __restrict__ h, T* __restrict__ g, const unsigned* __restri
     // ---- pulls ------------------------------------------------------------------------------------
     // f_i(x) = h_i(x - c_i), or h_opp(i)(x) across a solid link
     auto src_of = [&](int k, int i, const long long (&zoff)[3], long long n, unsigned lk) -> const T* {
-        const T* base = h + (long long)(k * Q) * NP;
-        if (HAS_SOLID && i > 0 && (lk >> dir_opp(i) & 1u)) return base + (long long)dir_opp(i) * NP + n;
-        return base + (long long)i * NP + zoff[1 - dir_cz(i)] + ys[1 - dir_cy(i)] + xs[1 - dir_cx(i)];
+        if (HAS_SOLID && i > 0 && (lk >> dir_opp(i) & 1u)) return h + (long long)pop_plane(k, dir_opp(i)) * NP + n;
+        return h + (long long)pop_plane(k, i) * NP + zoff[1 - dir_cz(i)] + ys[1 - dir_cy(i)] + xs[1 - dir_cx(i)];
     };
     auto plane_of = [&](int p, long long (&zoff)[3], long long& n, unsigned& lk) {
         zoff[0] = wrapz(p - 1) * pl; zoff[1] = wrapz(p) * pl; zoff[2] = wrapz(p + 1) * pl;
@@ -375,11 +374,11 @@ k_step_pull(const T* __restrict__ h, T* __restrict__ g, const unsigned* __restri
             const T omc = T(1) - om_b;
             const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
             const T ae = T(1) - T(1.5) * (eb[0] * eb[0] + eb[1] * eb[1] + eb[2] * eb[2]);
-            T* o = g + (long long)Q * NP + n;
+            T* o = g + n;
             T bs = T(0);
             {
                 const T h0 = fluid ? omc * stash[t] + w_rest<T>() * rb * (ae - omc * a0) : zero;
-                if (fluid && store_h) o[0] = h0;
+                if (fluid && store_h) o[(long long)pop_plane(1, 0) * NP] = h0;
                 u0b[1] = h0;
             }
 #pragma unroll
@@ -393,7 +392,7 @@ k_step_pull(const T* __restrict__ h, T* __restrict__ g, const unsigned* __restri
                     const T asym = (T(3) * wr) * (ce - omc * cu);
                     h1 = omc * stash[(2 * p + 1) * NT + t] + (sym + asym);
                     h2 = omc * stash[(2 * p + 2) * NT + t] + (sym - asym);
-                    if (store_h) { o[(long long)(2 * p + 1) * NP] = h1; o[(long long)(2 * p + 2) * NP] = h2; }
+                    if (store_h) { o[(long long)pop_plane(1, 2 * p + 1) * NP] = h1; o[(long long)pop_plane(1, 2 * p + 2) * NP] = h2; }
                     if (HAS_SOLID) {                             // bounced-back arrivals of the next step come from this node
                         if (lk >> (2 * p + 1) & 1u) bs += h1;
                         if (lk >> (2 * p + 2) & 1u) bs += h2;
@@ -415,7 +414,7 @@ k_step_pull(const T* __restrict__ h, T* __restrict__ g, const unsigned* __restri
                 collide19<T>(fr, rr, T(1) - om_r, ux, uy, uz, er[0], er[1], er[2]);
                 if (store_h) {
 #pragma unroll
-                    for (int i = 0; i < Q; ++i) g[(long long)i * NP + n] = fr[i];
+                    for (int i = 0; i < Q; ++i) g[(long long)pop_plane(0, i) * NP + n] = fr[i];
                 }
                 if (HAS_SOLID) {
 #pragma unroll
