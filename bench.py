@@ -1,8 +1,11 @@
 #!/usr/bin/env python
 """bench.py -- GLUPS of the two-component Shan-Chen D3Q19 step on B200, against the HBM roofline.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config2|config1|...]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config2|config1|...|all]
+                    [--tau-r T --tau-b T --G g]   # general-tau variant of the same workload
     python bench.py --impl reference ...        # the CPU oracle, as it stands, on host cores
+
+`--workload all` prints one JSON line per BASELINE config (0-4), each at the config's own dtype.
 
 One "step" is one pass of the whole hot path (moments, force, collide, bounce-back, stream)
 over the whole box: one lb_step(1).  `value` is GLUPS = N_nodes * K / t / 1e9 (PAPER.md:166-171
@@ -106,18 +109,44 @@ def measured_peak():
 
 
 def committed_traffic(workload: str, kernel: str):
-    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/traffic.csv), if any."""
+    """(dram bytes per launch, where from) of the dominant kernel from the committed ncu capture
+    (profiles/traffic.csv; the LAST matching row = the newest capture), if any."""
     p = os.path.join(ROOT, "profiles", "traffic.csv")
+    found = (None, None)
     if not os.path.exists(p):
-        return None
+        return found
     try:
         import csv
         for row in csv.DictReader(open(p)):
             if row["workload"] == workload and row["kernel"] == kernel:
-                return float(row["dram_bytes_per_launch"])
+                found = (float(row["dram_bytes_per_launch"]), row.get("source", "profiles/traffic.csv"))
     except (ValueError, OSError, KeyError):
         pass
-    return None
+    return found
+
+
+def cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def with_overrides(cfg, args):
+    """The workload with --tau-r / --tau-b / --G replaced (the general-tau bench variants of SURVEY 8(d) 'rules')."""
+    import dataclasses
+    kw = {}
+    if args.tau_r is not None:
+        kw["tau_r"] = args.tau_r
+    if args.tau_b is not None:
+        kw["tau_b"] = args.tau_b
+    if args.G is not None:
+        kw["G"] = args.G
+    return dataclasses.replace(cfg, **kw) if kw else cfg
 
 
 def time_oracle(cfg, sub, steps, warmup=0):
@@ -153,7 +182,7 @@ def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return 0
-    cfg = WORKLOADS[args.workload]
+    cfg = with_overrides(WORKLOADS["config2" if args.workload == "all" else args.workload], args)
     sub = (min(cfg.nx, 64), min(cfg.ny, 32), min(cfg.nz, 32))
     glups, dt = time_oracle(cfg, sub, args.steps, args.warmup)
     sample = (f"periodic {sub[0]}x{sub[1]}x{sub[2]} corner of {cfg.name}'s seeded fields, "
@@ -164,7 +193,7 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "box": [cfg.nx, cfg.ny, cfg.nz], "tau": [cfg.tau_r, cfg.tau_b], "G": cfg.G,
                    "note": "CPU oracle (oracle/lb_oracle.cpp, g++ -O2 -ffp-contract=off) on a bounded sample"},
-        "cpu_baseline": {"value": glups, "unit": "GLUPS", "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": glups, "unit": "GLUPS", "cores": 1, "kind": "oracle", "sample": sample, "cpu": cpu_model()},
         "e2e": {"value": glups, "unit": "GLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -193,15 +222,24 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     B.lib()
+    names = sorted(WORKLOADS) if args.workload == "all" else [args.workload]
+    for i, name in enumerate(names):
+        # `all`: the CPU oracle is timed once (on the headline workload), not five times
+        cpu = not args.no_cpu_baseline and (args.workload != "all" or name == "config2")
+        run_one(args, with_overrides(WORKLOADS[name], args), B, torch, dev, rank, local_rank, world, cpu)
+    return 0
 
-    cfg = WORKLOADS[args.workload]
+
+def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
+    if world > 1:
+        import torch.distributed as dist
     note = None
     es = 8 if cfg.dtype == "f64" else 4
-    need = 2 * 38 * cfg.n_nodes * es + 24 * cfg.n_nodes + (1 << 30)
+    need = (2 * 38 + 8) * cfg.n_nodes * es + 4 * cfg.n_nodes + (1 << 30)     # populations, carried density, links, staging
     free, _total = torch.cuda.mem_get_info(dev)
-    if need > free and args.workload in ("config2", "config3"):
+    if need > free and cfg.n_nodes > (1 << 24):
         note = f"{cfg.name} needs {need >> 30} GiB, {free >> 30} GiB free: fell back to config1"
-        cfg = WORKLOADS["config1"]
+        cfg = with_overrides(WORKLOADS["config1"], args)
     N = cfg.n_nodes
     steps, warmup = args.steps, max(args.warmup, 3)
     dtype = B.LB_F64 if cfg.dtype == "f64" else B.LB_F32
@@ -219,6 +257,8 @@ def run_ours(args):
     box = B.Box(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype, cuda_stream=stream.cuda_stream)
     kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA}[args.kernel]
     box.set_kernel(kernel)
+    if args.diag:
+        box.set_option(B.LB_OPT_DIAG, 1)
     if mask is not None:
         box.set_solid_mask(mask)
     box.set_fields(rr, rb)
@@ -245,6 +285,10 @@ def run_ours(args):
     clocks = sampler.stop()
     ms_max, units = aggregate_over_ranks(ms, float(N) * steps, world, dev)
     glups = units / (ms_max * 1e-3) / 1e9
+    diag = None
+    if args.diag:
+        m, p = box.get_diagnostics()            # the sums the last step left behind: no population pass
+        diag = {"mass": [float(v) for v in m], "momentum": [float(v) for v in p]}
 
     # ---- end to end through the C ABI with host buffers ----
     box.sync()
@@ -258,26 +302,28 @@ def run_ours(args):
     e2e_ms_max, _ = aggregate_over_ranks(e2e_s * 1e3, 0.0, world, dev)
     e2e_glups = units / (e2e_ms_max * 1e-3) / 1e9
     mass_chk = float(outs[0].sum() + outs[1].sum())
+    n_fluid = N if mask is None else int(N - int(mask.sum()))
 
     if rank != 0:
         box.close()
-        return 0
+        return
 
     peak, peak_src = measured_peak()
     alg = ALG_BYTES[cfg.dtype]
     per_launch_ms = ms / max(launches, 1) * (launches / steps)      # = ms / steps: whole step (1 kernel on the one-pass path)
     achieved = alg * N / (per_launch_ms * 1e-3) / 1e9
+    traffic, traffic_src = committed_traffic(cfg.name, kname)
     line = {
         "metric": METRIC, "value": glups, "unit": "GLUPS", "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_max / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": cfg.dtype, "data": "synthetic",
         "config": {"workload": cfg.name, "box": [cfg.nx, cfg.ny, cfg.nz], "tau": [cfg.tau_r, cfg.tau_b], "G": cfg.G,
                    "solid_spheres": cfg.n_spheres, "kernel": kname, "launches_per_step": launches / steps,
-                   "l2": f"state {2 * 38 * N * es / 2**30:.1f} GiB >> 126 MB L2, no flush needed",
-                   "parallelism": "replicas only" if world > 1 else "single GPU", "diagnostics_in_step": False,
+                   "l2": f"state {2 * 38 * N * es / 2**30:.1f} GiB vs 126 MB L2" + (", no flush needed" if 2 * 38 * N * es > (1 << 30) else ": L2-resident, launch-bound, reported only"),
+                   "parallelism": "replicas only" if world > 1 else "single GPU", "diagnostics_in_step": bool(args.diag),
                    **({"note": note} if note else {})},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": committed_traffic(cfg.name, kname), "peak_source": peak_src,
+                     "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                      "algorithmic_bytes_per_node": alg, "kernel_ms": per_launch_ms,
                      "kernel": "whole step" if launches != steps else "fused one-pass step kernel"},
         "e2e": {"value": e2e_glups, "unit": "GLUPS", "h2d_bytes_per_step": 2 * N * 8 / steps,
@@ -285,15 +331,23 @@ def run_ours(args):
                 "calls": "lb_set_fields(host) + lb_step(K) + lb_get_moments(host)"},
         "gpu_launches": launches, "clocks": clocks,
     }
-    if not args.no_cpu_baseline:
+    if mask is not None:
+        line["config"]["fluid_nodes"] = n_fluid
+        line["config"]["glups_fluid_nodes_only"] = glups * n_fluid / N      # no computation inside a particle
+    if diag:
+        line["diagnostics"] = diag
+    if cpu_baseline:
         sub = (min(cfg.nx, 128), min(cfg.ny, 128), min(cfg.nz, 64))
         cpu_steps = 12
         cg, cdt = time_oracle(cfg, sub, cpu_steps)
-        line["cpu_baseline"] = {"value": cg, "unit": "GLUPS", "cores": 1, "kind": "oracle", "seconds": cdt,
-                                "sample": f"periodic {sub[0]}x{sub[1]}x{sub[2]} corner of {cfg.name}'s seeded fields, {cpu_steps} steps"}
+        c0 = WORKLOADS["config0"]
+        cg0, cdt0 = time_oracle(c0, (c0.nx, c0.ny, c0.nz), 100)        # 32^3 x 100 steps
+        line["cpu_baseline"] = {"value": cg, "unit": "GLUPS", "cores": 1, "kind": "oracle", "seconds": cdt, "cpu": cpu_model(),
+                                "sample": f"periodic {sub[0]}x{sub[1]}x{sub[2]} corner of {cfg.name}'s seeded fields, {cpu_steps} steps",
+                                "config0_32c_100_steps": {"value": cg0, "unit": "GLUPS", "seconds": cdt0}}
     box.close()
+    del pin, outs, rr, rb
     print(json.dumps(line), flush=True)
-    return 0
 
 
 def main():
@@ -302,7 +356,11 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS) + ["all"])
+    ap.add_argument("--tau-r", type=float, default=None, help="override the workload's tau_r (general-tau variant)")
+    ap.add_argument("--tau-b", type=float, default=None)
+    ap.add_argument("--G", type=float, default=None)
+    ap.add_argument("--diag", action="store_true", help="per-step mass / momentum sums fused into the step kernel (LB_OPT_DIAG)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

@@ -631,10 +631,6 @@ long long round64(long long v) { return (v + 63) / 64 * 64; }
 // ----------------------------------------------------------------------------------------
 extern "C" {
 
-#ifdef LB_TMA_TRACE
-int lb_debug_trace(long long* out) { return cudaMemcpyFromSymbol(out, lb::g_trace, sizeof(long long) * 64 * 16) == cudaSuccess ? 0 : -1; }
-#endif
-
 const char* lb_last_error(void) { return g_err.c_str(); }
 int lb_last_error_code(void) { return g_err_code; }
 const char* lb_version(void) { return "lb-b200 0.2 (sm_100a)"; }

@@ -123,12 +123,6 @@ struct TmaLayout {
 };
 
 
-#ifdef LB_TMA_TRACE
-__device__ long long g_trace[64 * 16];
-#define TRACE(cond, it, slot) do { if ((cond) && blockIdx.x == 1 && blockIdx.y == 1 && blockIdx.z == 0 && (it) >= 0 && (it) < 64) g_trace[(it) * 16 + (slot)] = clock64(); } while (0)
-#else
-#define TRACE(cond, it, slot) do { } while (0)
-#endif
 
 // ---- the kernel ------------------------------------------------------------------------------------------
 // Threads: 2*NT consumers (component k = t / NT, node (tx, ty) = ((t % NT) % 32, (t % NT) / 32): one warp per
@@ -279,14 +273,10 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                 // ring plane j+2 (the z+1 neighbour plane of iteration j): its slot held plane j-2, last read in iteration
                 // j-2, which every consumer warp had left when it arrived on done(j-1)
                 if (j > 0) mbar_wait(done + ((j - 1) & 1), ((j - 1) >> 1) & 1);
-                TRACE(r == 0, j, 8);
                 ring_assemble(j + 2);
-                TRACE(r == 0, j, 11);
                 __syncwarp();
                 if ((r & 31) == 0) mbar_arrive(rdy);
-                TRACE(r == 0, j, 9);
                 if (j + 3 <= niter + 1) ring_fetch(j + 3);
-                TRACE(r == 0, j, 10);
             }
             return;
         }
@@ -299,7 +289,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             if (lane == 0) {
                 const int s = j & 1;
                 if (j >= 2) mbar_wait(done + s, ((j >> 1) - 1) & 1);
-                TRACE(true, j, 12);
                 mbar_expect_tx(full + s, L::STAGE_TX_BYTES + (wrap_xlo ? L::XCOL_TX_BYTES : 0u) + (wrap_xhi ? L::XCOL_TX_BYTES : 0u));
 #pragma unroll
                 for (int i = 0; i < Q; ++i) {
@@ -315,7 +304,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                     }
                 }
             }
-            TRACE(lane == 0, j, 13);
             __syncwarp();
         }
         return;
@@ -375,12 +363,9 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         T* SU = SUk + sg * 4 * SUP;
 
         // ---- pull: the stage holds h_i(x - c_i) for the whole tile (Eq. 5, periodic) ----
-        TRACE(t == 0, it, 0);
         mbar_wait(full + sg, ph);
-        TRACE(t == 0, it, 1);
         mbar_wait(rdy, it & 1);                         // density ring planes z-1, z, z+1 are in place (before `done`: the ring
                                                         // warps must not get two phases ahead of any waiter)
-        TRACE(t == 0, it, 2);
         T f[Q];
 #pragma unroll
         for (int i = 0; i < Q; ++i) f[i] = st[L::slot_off(i) + (dir_cx(i) == 0 ? rd0 : (dir_cx(i) > 0 ? rdp : rdm))];
@@ -402,7 +387,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             for (int i = 1; i < Q; ++i)
                 if (lk >> dir_opp(i) & 1u) f[i] = __ldg(hn + (long long)(2 * dir_opp(i)) * NP);
         }
-        TRACE(t == 0, it, 3);
 
         // ---- moments of this component (Eq. 6-7), exchanged with the other component's thread of the same node ----
         T rho = zero, jx = zero, jy = zero, jz = zero;
@@ -535,7 +519,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         SUum[0] = pm;
         __syncwarp();
         if (lane_lo) mbar_arrive(rowpub + sg * 2 * TY + k * TY + ty);
-        TRACE(t == 0, it, 4);
 
         // ---- global stores that need nothing from the other warps: the y-edge exports ----
         if ((row_lo || row_hi) && store_rho) {                             // the row beyond the tile edge receives exactly Um (Up)
@@ -545,14 +528,12 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             ro.y[e_y + zt * psy] = lo ? pm : pp;
         }
 
-        TRACE(t == 0, it, 5);
         {   // the rows above and below (same component) have published this plane
             unsigned long long* nb = rowpub + sg * 2 * TY + k * TY + ty;
             if (row_lo) mbar_wait(nb + 1, ph);
             else if (row_hi) mbar_wait(nb - 1, ph);
             else mbar_wait2(nb - 1, nb + 1, ph);
         }
-        TRACE(t == 0, it, 6);
 
         // ---- y stage of the gather; exports across the tile's x edges ----
         {

@@ -24,7 +24,19 @@ def _built():
 
 
 def nerr(a, b):
+    """Reading S12: max|a - b| / max|b| over all populations (global-max normalisation)."""
     return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+_W19 = np.array([1 / 3] + [1 / 18] * 6 + [1 / 36] * 12)
+
+
+def perr(a, b):
+    """Per-element relative error with the floor |b| >= 1e-3 w_i ('for information'): a, b [2][19][...]."""
+    a = a.reshape(2, 19, -1)
+    b = b.reshape(2, 19, -1)
+    floor = 1e-3 * _W19[None, :, None]
+    return float((np.abs(a - b) / np.maximum(np.abs(b), floor)).max())
 
 
 def make_box(nx, ny, nz, kernel, **kw):
@@ -71,10 +83,14 @@ def test_config0_100_steps_fp64(oracle_mod, kernel):
         for t in (1, 2, 10, 50, 100):
             o.step(t - done), box.step(t - done)
             done = t
-            e = nerr(box.get_populations(), o.get_populations())
+            fg, fo = box.get_populations(), o.get_populations()
+            e, pe = nerr(fg, fo), perr(fg, fo)
             worst = max(worst, e)
-            print(f"config0 {KNAME[kernel]} t={t}: normalised max err {e:.3e}")
+            print(f"config0 {KNAME[kernel]} t={t}: normalised max err {e:.3e}, per element {pe:.3e}")
+            if t <= 50:
+                assert pe < 1e-11                                # per element too while no population has crossed zero (S12)
         assert worst < 1e-11                                     # north_star bar
+        assert pe < 1e-8                                         # t = 100: populations cross zero (S12: two fp64 codes differ by 7e-11)
         # same binary, same inputs: moments and diagnostics agree with the oracle too
         gm, om = box.get_moments(), o.get_moments()
         for a in range(5):
@@ -173,69 +189,121 @@ def test_wall_and_single_solid_node(oracle_mod, kernel):
 
 
 # ---------------------------------------------------------------------------------------------
-# fp32 variant
+# fp32 variant (north_star: "fp32: within 1e-4 relative"; reading S12-fp32 in DESIGN.md section 3)
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
-def test_fp32_against_fp64_oracle(oracle_mod, kernel):
-    cfg = w.CONFIGS[0]
-    rr, rb = cfg.fields()
-    o = oracle_mod.Oracle(cfg.nx, cfg.ny, cfg.nz)
-    o.set_fields(rr, rb)
-    with make_box(cfg.nx, cfg.ny, cfg.nz, kernel, dtype=B.LB_F32) as box:
+def _fp32_run(kernel, cfg, rr, rb, horizons, G=None):
+    out = {}
+    with make_box(cfg.nx, cfg.ny, cfg.nz, kernel, tau_r=cfg.tau_r, tau_b=cfg.tau_b, G=cfg.G if G is None else G, dtype=B.LB_F32) as box:
         box.set_fields(rr, rb)
         done = 0
-        for t in (1, 10, 50, 100):
-            o.step(t - done), box.step(t - done)
+        for t in horizons:
+            box.step(t - done)
             done = t
-            e = nerr(box.get_populations(), o.get_populations())
-            print(f"fp32 {KNAME[kernel]} t={t}: normalised max err {e:.3e}")
-            if t <= 50:
-                assert e < 1e-4                                   # north_star bar
-        # t = 100 of config 0 amplifies rounding noise ~5500x (S12): report, bound loosely
-        assert e < 5e-3
-        m, p = box.get_diagnostics()
-        assert np.abs(m / np.array([rr.sum(), rb.sum()]) - 1).max() < 1e-5
+            out[t] = box.get_populations().copy()
+        out["diag"] = box.get_diagnostics()
+    return out
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_fp32_against_fp64_oracle(oracle_mod, kernel):
+    """Config 0 in fp32 against the fp64 oracle.  The bar is 1e-4 (normalised, S12) wherever two correct fp32
+    codes can meet it: up to t = 50.  Config 0 is a linear instability (S12): by t = 100 it has amplified rounding
+    differences ~5500 x, so there the bar is the MEASURED fp32 noise floor -- the distance between two fp32
+    formulations of the same update (this kernel and the two-pass kernel, different summation orders) -- times 4."""
+    cfg = w.CONFIGS[0]
+    rr, rb = cfg.fields()
+    horizons = (1, 10, 50, 100)
+    o = oracle_mod.Oracle(cfg.nx, cfg.ny, cfg.nz)
+    o.set_fields(rr, rb)
+    want, done = {}, 0
+    for t in horizons:
+        o.step(t - done)
+        done = t
+        want[t] = o.get_populations().copy()
+    got = _fp32_run(kernel, cfg, rr, rb, horizons)
+    other = _fp32_run(B.LB_KERNEL_TWOPASS if kernel != B.LB_KERNEL_TWOPASS else B.LB_KERNEL_TMA, cfg, rr, rb, horizons)
+    for t in horizons:
+        e = nerr(got[t], want[t])
+        floor = nerr(got[t], other[t])
+        print(f"fp32 {KNAME[kernel]} t={t}: normalised max err vs fp64 oracle {e:.3e}; fp32-vs-fp32 floor {floor:.3e}")
+        if t <= 50:
+            assert e < 1e-4                                       # north_star bar
+        else:
+            assert e < max(1e-4, 4 * floor) and e < 5e-3
+    m, p = got["diag"]
+    assert np.abs(m / np.array([rr.sum(), rb.sum()]) - 1).max() < 1e-5
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KNAME.get)
+def test_fp32_stable_mixture_100_steps(oracle_mod, kernel):
+    """The same box below the demixing threshold (G = 0.4, pin P10: perturbations decay): nothing amplifies the
+    rounding noise, and fp32 stays within the north_star bar of 1e-4 over the full 100 steps."""
+    cfg = w.CONFIGS[0]
+    rr, rb = cfg.fields()
+    o = oracle_mod.Oracle(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, 0.4)
+    o.set_fields(rr, rb)
+    o.step(100)
+    got = _fp32_run(kernel, cfg, rr, rb, (100,), G=0.4)
+    e = nerr(got[100], o.get_populations())
+    print(f"fp32 {KNAME[kernel]} stable mixture t=100: normalised max err {e:.3e}")
+    assert e < 1e-4
 
 
 # ---------------------------------------------------------------------------------------------
-# full-size box, the configuration bench.py times: sampled outputs + invariants
+# full-size boxes, the configurations bench.py times: sampled outputs + invariants
 # ---------------------------------------------------------------------------------------------
-def _sample_points(nx, ny, nz, k=24):
+S_FULL, HW_FULL = 10, 21        # after s steps a node depends on the initial state within 2 s nodes: cut-out half width 2 s + 1
+
+
+def _sample_points(nx, ny, nz, k=24, zc=None):
     rng = np.random.default_rng(99)
     pts = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (0, ny - 1, 5), (31, 7, 0), (32, 8, nz - 1), (nx - 1, 0, nz // 2)]
+    if zc:                                                       # both sides of a z-chunk seam, on a tile corner
+        pts += [(63, 15, zc - 1), (64, 16, zc), (nx - 1, 8, 2 * zc - 1 if 2 * zc <= nz else zc - 1), (0, 7, zc % nz)]
     pts += [tuple(int(v) for v in rng.integers(0, (nx, ny, nz))) for _ in range(k - len(pts))]
     return pts
 
 
-@pytest.mark.parametrize("cfg_idx,dtype,tol", [(1, B.LB_F64, 1e-13), (1, B.LB_F32, 2e-6)])
+def _cutout_oracle(oracle_mod, cfg, R, Bl, M, x, y, z, s, hw):
+    """The oracle on the periodic (2 hw + 1)^3 cut-out of the SAME seeded initial fields (and mask) around (x, y, z)."""
+    ix = np.arange(x - hw, x + hw + 1) % cfg.nx
+    iy = np.arange(y - hw, y + hw + 1) % cfg.ny
+    iz = np.arange(z - hw, z + hw + 1) % cfg.nz
+    sub = np.ix_(iz, iy, ix)
+    L = 2 * hw + 1
+    o = oracle_mod.Oracle(L, L, L, cfg.tau_r, cfg.tau_b, cfg.G)
+    if M is not None:
+        o.set_solid_mask(np.ascontiguousarray(M[sub]).reshape(-1))
+    o.set_fields(np.ascontiguousarray(R[sub]).reshape(-1), np.ascontiguousarray(Bl[sub]).reshape(-1))
+    o.step(s)
+    return o
+
+
+@pytest.mark.parametrize("cfg_idx,dtype,tol", [(1, B.LB_F64, 1e-13), (1, B.LB_F32, 1e-5)])
 def test_full_size_sampled_outputs_and_invariants(oracle_mod, cfg_idx, dtype, tol):
-    """256^3 (bench workload).  After s steps a node depends on the initial fields within 2s
-    nodes, so the oracle can compute any sampled node from a (4s+3)^3 cut-out of the SAME
-    seeded initial fields."""
+    """256^3 (bench workload, default kernel and launch configuration), all 38 populations at sampled nodes after 10 steps."""
     cfg = w.CONFIGS[cfg_idx]
     nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
-    s, hw = 3, 7
+    s, hw = S_FULL, HW_FULL
     rr, rb = cfg.fields()
     R, Bl = rr.reshape(nz, ny, nx), rb.reshape(nz, ny, nx)
     with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype) as box:
+        assert B.lb_kernel_name(box.h) == "tma"
         box.set_fields(rr, rb)
         m0, p0 = box.get_diagnostics()
         box.step(s)
         f = box.get_populations()
-        for (x, y, z) in _sample_points(nx, ny, nz):
-            ix = np.arange(x - hw, x + hw + 1) % nx
-            iy = np.arange(y - hw, y + hw + 1) % ny
-            iz = np.arange(z - hw, z + hw + 1) % nz
-            sub = np.ix_(iz, iy, ix)
-            L = 2 * hw + 1
-            o = oracle_mod.Oracle(L, L, L, cfg.tau_r, cfg.tau_b, cfg.G)
-            o.set_fields(R[sub].reshape(-1), Bl[sub].reshape(-1))
-            o.step(s)
+        worst = 0.0
+        for (x, y, z) in _sample_points(nx, ny, nz, zc=box.get_option(B.LB_OPT_ZC)):
+            o = _cutout_oracle(oracle_mod, cfg, R, Bl, None, x, y, z, s, hw)
             want = o.get_populations()[:, :, hw, hw, hw]
             got = f[:, :, z, y, x]
-            assert np.abs(got - want).max() / np.abs(want).max() < tol, (x, y, z)
+            e = np.abs(got - want).max() / np.abs(want).max()
+            worst = max(worst, e)
+            assert e < tol, (x, y, z)
+        print(f"{cfg.name} dtype {dtype}: worst sampled normalised error after {s} steps {worst:.3e}")
         del f
-        box.step(47)
+        box.step(40)
         m1, p1 = box.get_diagnostics()
         if dtype == B.LB_F64:
             assert np.abs(m1 / m0 - 1).max() < 1e-13             # per-component mass
@@ -244,58 +312,98 @@ def test_full_size_sampled_outputs_and_invariants(oracle_mod, cfg_idx, dtype, to
             assert np.abs(m1 / m0 - 1).max() < 1e-5
 
 
-def test_headline_512_cube_sampled_moments_and_invariants(oracle_mod):
-    """Config 2 (512^3 fp64, the workload bench.py times by default, same kernel and launch configuration).
+def test_config4_spheres_full_size_sampled_populations(oracle_mod):
+    """Config 4 (256^3, 2000 spheres R = 5.5; bounce-back PAPER.md:412-421) at the size and in the launch configuration
+    bench.py times: all 38 populations after 10 steps at nodes next to sphere surfaces, at tile / z-chunk seams and at
+    random places, against the oracle on a cut-out of the same fields AND the same mask; then per-component mass."""
+    cfg = w.CONFIGS[4]
+    nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
+    s, hw = S_FULL, HW_FULL
+    rr, rb = cfg.fields()
+    mask = cfg.solid_mask()
+    R, Bl, M = rr.reshape(nz, ny, nx), rb.reshape(nz, ny, nx), mask.reshape(nz, ny, nx)
+    with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G) as box:
+        assert B.lb_kernel_name(box.h) == "tma"
+        box.set_solid_mask(mask)
+        box.set_fields(rr, rb)
+        zc = box.get_option(B.LB_OPT_ZC)
+        links = box.get_link_mask().reshape(nz, ny, nx)
+        m0, _ = box.get_diagnostics()
+        box.step(s)
+        f = box.get_populations()
+        # fluid nodes with bounce-back links: some anywhere, some on z-chunk seams and tile edges
+        rng = np.random.default_rng(4)
+        zs, ys, xs = np.nonzero(links)
+        pick = rng.choice(zs.size, 10, replace=False)
+        pts = [(int(xs[i]), int(ys[i]), int(zs[i])) for i in pick]
+        seam = np.nonzero((links != 0) & ((np.arange(nz) % zc == 0) | (np.arange(nz) % zc == zc - 1))[:, None, None])
+        pick = rng.choice(seam[0].size, 5, replace=False)
+        pts += [(int(seam[2][i]), int(seam[1][i]), int(seam[0][i])) for i in pick]
+        edge = np.nonzero((links != 0) & ((np.arange(nx) % 32 == 0) | (np.arange(nx) % 32 == 31))[None, None, :]
+                          & ((np.arange(ny) % 8 == 0) | (np.arange(ny) % 8 == 7))[None, :, None])
+        pick = rng.choice(edge[0].size, 5, replace=False)
+        pts += [(int(edge[2][i]), int(edge[1][i]), int(edge[0][i])) for i in pick]
+        pts += [p for p in _sample_points(nx, ny, nz, k=12, zc=zc)]
+        worst, n_solid = 0.0, 0
+        for (x, y, z) in pts:
+            got = f[:, :, z, y, x]
+            if M[z, y, x]:
+                n_solid += 1
+                assert np.all(got == 0.0), (x, y, z)             # S8: exactly zero, never written
+                continue
+            o = _cutout_oracle(oracle_mod, cfg, R, Bl, M, x, y, z, s, hw)
+            want = o.get_populations()[:, :, hw, hw, hw]
+            e = np.abs(got - want).max() / np.abs(want).max()
+            worst = max(worst, e)
+            assert e < 1e-13, (x, y, z)
+        print(f"{cfg.name}: {len(pts) - n_solid} fluid sample nodes (20 with links), worst normalised error after {s} steps {worst:.3e}")
+        assert np.all(f[:, :, M == 1] == 0.0)
+        del f
+        box.step(40)
+        m1, _ = box.get_diagnostics()
+        assert np.abs(m1 / m0 - 1).max() < 1e-13                 # per-component mass with bounce-back (pin P2)
+
+
+@pytest.mark.parametrize("cfg_idx,dtype,tols", [(2, B.LB_F64, (1e-13, 1e-16)), (3, B.LB_F32, (2e-6, 2e-7))])
+def test_headline_512_cube_sampled_moments_and_invariants(oracle_mod, cfg_idx, dtype, tols):
+    """Configs 2 and 3 (512^3 fp64 / fp32, the workloads bench.py times, same kernel and launch configuration).
     The 38 x 1 GiB populations are not brought to the host: rho_r, rho_b, u (Eq. 6-7, which sum all 38 of them)
     are compared at sampled nodes with the oracle run on a cut-out of the SAME seeded initial fields, and the
     conserved sums are followed over more steps."""
     import torch
-    cfg = w.CONFIGS[2]
+    cfg = w.CONFIGS[cfg_idx]
     nx, ny, nz = cfg.nx, cfg.ny, cfg.nz
-    need = 2 * 38 * cfg.n_nodes * 8 + 64 * cfg.n_nodes
+    es = 8 if dtype == B.LB_F64 else 4
+    need = 2 * 38 * cfg.n_nodes * es + 64 * cfg.n_nodes
     if torch.cuda.mem_get_info()[0] < need:
-        pytest.skip("not enough free device memory for 512^3 fp64")
-    s, hw = 3, 7
+        pytest.skip("not enough free device memory for 512^3")
+    s, hw = S_FULL, HW_FULL
     rr, rb = cfg.fields()
     R, Bl = rr.reshape(nz, ny, nx), rb.reshape(nz, ny, nx)
-    with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G) as box:
+    with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype) as box:
         assert B.lb_kernel_name(box.h) == "tma"
         box.set_fields(rr, rb)
         m0, p0 = box.get_diagnostics()
         box.step(s)
         got = [a.reshape(nz, ny, nx) for a in box.get_moments()]
-        for (x, y, z) in _sample_points(nx, ny, nz, k=16):
-            ix = np.arange(x - hw, x + hw + 1) % nx
-            iy = np.arange(y - hw, y + hw + 1) % ny
-            iz = np.arange(z - hw, z + hw + 1) % nz
-            sub = np.ix_(iz, iy, ix)
+        worst = [0.0, 0.0]
+        for (x, y, z) in _sample_points(nx, ny, nz, k=16, zc=box.get_option(B.LB_OPT_ZC)):
+            o = _cutout_oracle(oracle_mod, cfg, R, Bl, None, x, y, z, s, hw)
             L = 2 * hw + 1
-            o = oracle_mod.Oracle(L, L, L, cfg.tau_r, cfg.tau_b, cfg.G)
-            o.set_fields(R[sub].reshape(-1), Bl[sub].reshape(-1))
-            o.step(s)
             want = [a.reshape(L, L, L)[hw, hw, hw] for a in o.get_moments()]
-            for gq, wq, scale in zip(got, want, (1.0, 1.0, 1e-3, 1e-3, 1e-3)):
-                assert abs(gq[z, y, x] - wq) < 1e-13 * scale + 1e-15, (x, y, z)
+            for q, (gq, wq) in enumerate(zip(got, want)):
+                d = abs(gq[z, y, x] - wq)
+                worst[q >= 2] = max(worst[q >= 2], d)
+                assert d < tols[q >= 2], (x, y, z, q)            # densities ~ 1, velocities ~ 1e-3
+        print(f"{cfg.name}: worst sampled |rho - rho_ora| {worst[0]:.3e}, |u - u_ora| {worst[1]:.3e} after {s} steps")
         del got
-        box.step(17)
+        box.step(10)
         m1, p1 = box.get_diagnostics()
-        assert np.abs(m1 / m0 - 1).max() < 1e-13                 # per-component mass
-        assert np.abs(p1 - p0).max() < 1e-7                       # total momentum (|P| ~ 0, N = 1.3e8)
-
-
-def test_tma_kernel_with_32x4_tiles():
-    """LB_TMA_TY=4 selects the 32 x 4 tile / two CTAs per SM variant of the TMA kernel when the library creates a
-    context: the small-box, tile-edge and solid parity cases are run again under it in a child process."""
-    import os
-    import subprocess
-    import sys
-    if os.environ.get("LB_TMA_TY") == "4":
-        pytest.skip("already inside the child run")
-    env = dict(os.environ, LB_TMA_TY="4")
-    sel = "tma and (random_populations or ragged or spheres_64 or wall_and_single)"
-    r = subprocess.run([sys.executable, "-m", "pytest", os.path.abspath(__file__), "-m", "gpu", "-x", "-q", "-k", sel],
-                       env=env, capture_output=True, text=True, timeout=600)
-    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+        if dtype == B.LB_F64:
+            assert np.abs(m1 / m0 - 1).max() < 1e-13             # per-component mass
+            assert np.abs(p1 - p0).max() < 1e-7                   # total momentum (|P| ~ 0, N = 1.3e8)
+        else:
+            assert np.abs(m1 / m0 - 1).max() < 1e-5
 
 
 # ---------------------------------------------------------------------------------------------
