@@ -255,7 +255,7 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
 
     stream = torch.cuda.Stream(device=dev)
     box = B.Box(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype, cuda_stream=stream.cuda_stream)
-    kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA}[args.kernel]
+    kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA, "halo": B.LB_KERNEL_HALO}[args.kernel]
     box.set_kernel(kernel)
     if args.diag:
         box.set_option(B.LB_OPT_DIAG, 1)
@@ -361,7 +361,7 @@ def main():
     ap.add_argument("--tau-b", type=float, default=None)
     ap.add_argument("--G", type=float, default=None)
     ap.add_argument("--diag", action="store_true", help="per-step mass / momentum sums fused into the step kernel (LB_OPT_DIAG)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma", "halo"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     return run_reference(args) if args.impl == "reference" else run_ours(args)

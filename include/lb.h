@@ -44,8 +44,8 @@ typedef struct lb_ctx lb_ctx;          /* opaque; owned by the library */
 
 enum { LB_OK = 0, LB_EINVAL = -1, LB_ENOMEM = -2, LB_ECUDA = -3, LB_ESTATE = -4 };
 enum { LB_F64 = 0, LB_F32 = 1 };
-enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2, LB_KERNEL_TMA = 3 };
-enum { LB_OPT_ZC = 1 };                /* options of lb_set_option */
+enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2, LB_KERNEL_TMA = 3, LB_KERNEL_HALO = 4 };
+enum { LB_OPT_ZC = 1, LB_OPT_DIAG = 2, LB_OPT_CLUSTER = 3 };   /* options of lb_set_option */
 
 /* Create a context for an nx*ny*nz periodic box holding two fluids with BGK
  * relaxation times tau_r, tau_b (Eq. 1; omega_k = 1/tau_k) coupled by the

@@ -16,8 +16,8 @@ import numpy as np
 
 LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 LB_F64, LB_F32 = 0, 1
-LB_KERNEL_AUTO, LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA = 0, 1, 2, 3
-LB_OPT_ZC = 1
+LB_KERNEL_AUTO, LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA, LB_KERNEL_HALO = 0, 1, 2, 3, 4
+LB_OPT_ZC, LB_OPT_DIAG, LB_OPT_CLUSTER = 1, 2, 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "_lib", "liblb_b200.so")
@@ -175,7 +175,7 @@ def lb_set_kernel(h, kind):
     _chk(lib().lb_set_kernel(h, kind))
 
 
-KERNEL_NAMES = {LB_KERNEL_TWOPASS: "twopass", LB_KERNEL_ONEPASS: "onepass", LB_KERNEL_TMA: "tma"}
+KERNEL_NAMES = {LB_KERNEL_TWOPASS: "twopass", LB_KERNEL_ONEPASS: "onepass", LB_KERNEL_TMA: "tma", LB_KERNEL_HALO: "halo"}
 
 
 def lb_kernel_name(h) -> str:

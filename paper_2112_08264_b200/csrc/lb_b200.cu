@@ -21,6 +21,7 @@
 #include "lb_lattice.cuh"
 #include "lb_onepass.cuh"
 #include "lb_tma.cuh"
+#include "lb_halo.cuh"
 
 using namespace lb;
 
@@ -42,8 +43,15 @@ struct lb_ctx {
     // rho_x / rho_y / rho_xy exist only when the box takes the one-pass tile.
     void* rho_in[2]; void* rho_x[2]; void* rho_y[2]; void* rho_xy[2];
     long long s_x, s_y, s_xy;   // component strides (elements) of the edge arrays
+    // the halo kernel (lb_halo.cuh): own-gather edge rows / columns (shapes of rho_y / rho_x), ping-pong with the others,
+    // and the x-halo copies of the populations, one per population buffer
+    void* rho_er[2]; void* rho_ec[2];
+    void* hx[2];
+    long long hx_elems;         // 20 * nz * (nx / 32) * ny
+    bool hx_valid;     // hx[cur] matches f[cur]
     int rcur;
-    bool rho_valid;    // rho_*[rcur] holds the density of the state in f[cur]
+    bool rho_valid;    // the density arrays [rcur] hold the density of the state in f[cur], in the format rho_fmt
+    int rho_fmt;       // RHO_FULL (rho_in + edge pieces: two-pass, one-pass, TMA kernels) or RHO_EDGE (frame arrays only: halo kernel)
     unsigned int* links;   // N words: bit i = neighbour i solid, bit 31 = this node solid
     bool has_solid;
     bool have_fields;
@@ -51,6 +59,13 @@ struct lb_ctx {
     int kernel_req;
     int zc;            // planes per CTA of the one-pass kernel
     int zc_tma;        // ... of the TMA kernel
+    CUtensorMap tmap_hx[2];   // [buffer] x-halo box TY x 1 x 1 x 2 over hx [plane][z][tile_x][y]
+    int cluster_x;     // LB_OPT_CLUSTER: thread-block cluster size along x for the TMA kernel (1 = none)
+    int diag_mode;     // LB_OPT_DIAG: the halo kernel also leaves the mass / momentum sums of the new state behind
+    bool diag_fresh;   // diag_cta holds the per-CTA partials of the state in f[cur]
+    double* diag_cta;  // [diag_cta_cap][5]
+    long long diag_cta_cap;
+    long long diag_ncta;
     CUtensorMap tmap[2][3];   // [buffer][narrow box 32 x 8, wide box (32 + 16 B) x 8, wrapped-column box 16 B x 8; each 2 planes deep] over [plane][z][y][x]
     bool have_tmap;
     double* stage;     // device staging, stage_nodes * 5 doubles
@@ -67,6 +82,7 @@ constexpr long long STAGE_NODES = 1ll << 22;
 constexpr int DIAG_BLOCKS = 148 * 8;
 constexpr unsigned SOLID_BIT = 1u << 31;
 constexpr int OP_TX = 32, OP_TY = 8;
+enum { RHO_FULL = 0, RHO_EDGE = 1 };
 
 thread_local std::string g_err;
 thread_local int g_err_code = LB_OK;
@@ -403,7 +419,8 @@ bool onepass_ok(const lb_ctx* c) { return c->nx % OP_TX == 0 && c->ny % OP_TY ==
 // rho_*[rcur] := density of the state in f[cur] (rho_in = the whole sum, the edge arrays zero)
 template <typename T>
 int ensure_rho(lb_ctx* c) {
-    if (c->rho_valid) return LB_OK;
+    if (c->rho_valid && c->rho_fmt == RHO_FULL) return LB_OK;
+    c->rho_fmt = RHO_FULL;
     const int r = c->rcur;
     if (c->rho_x[r]) {
         CU(cudaMemsetAsync(c->rho_x[r], 0, size_t(2) * c->s_x * sizeof(T), c->stream));
@@ -436,6 +453,8 @@ int step_twopass(lb_ctx* c) {
     CU(cudaGetLastError());
     c->cur ^= 1;
     c->rho_valid = false;
+    c->hx_valid = false;
+    c->diag_fresh = false;
     return LB_OK;
 }
 
@@ -455,6 +474,8 @@ int unstream_scratch(lb_ctx* c) {
     c->launches++;
     CU(cudaGetLastError());
     c->rho_valid = false;
+    c->hx_valid = false;
+    c->diag_fresh = false;
     return LB_OK;
 }
 
@@ -520,6 +541,8 @@ int step_onepass(lb_ctx* c) {
     if (rc != LB_OK) return rc;
     c->cur ^= 1;
     c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
+    c->hx_valid = false;
+    c->diag_fresh = false;
     return LB_OK;
 }
 
@@ -551,6 +574,15 @@ bool make_tmaps(lb_ctx* c) {
                     CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
                 return false;
         }
+    // x-halo arrays: dims (y', tile_x, z, plane 2 j + k), one box = the TY rows of one tile, both components
+    const cuuint64_t ntx = cuuint64_t(c->nx / OP_TX);
+    const cuuint64_t hdim[4] = {cuuint64_t(c->ny), ntx, cuuint64_t(c->nz), cuuint64_t(2 * NHALO)};
+    const cuuint64_t hstr[3] = {cuuint64_t(c->ny) * es, cuuint64_t(c->ny) * ntx * es, cuuint64_t(c->ny) * ntx * c->nz * es};
+    const cuuint32_t hbox[4] = {cuuint32_t(OP_TY), 1, 1, 2};
+    for (int b = 0; b < 2; ++b)
+        if (enc(&c->tmap_hx[b], dt, 4, c->hx[b], hdim, hstr, hbox, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+            return false;
     return true;
 }
 
@@ -560,6 +592,19 @@ int launch_tma(lb_ctx* c) {
     constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
     const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
+    if (c->cluster_x > 1 && grid.x % c->cluster_x == 0) {
+        // thread-block clusters along x: the CTAs of x-adjacent tiles start together, so the 16-byte box margins one of them reads
+        // are the other's own tile data of the same plane
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid; cfg.blockDim = dim3(2 * OP_TX * OP_TY + 128); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = unsigned(c->cluster_x); at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        CU(cudaLaunchKernelEx(&cfg, kern, c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
+                              static_cast<T*>(c->f[c->cur ^ 1]), static_cast<const unsigned*>(HAS_SOLID ? c->links : nullptr),
+                              rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz, c->zc_tma, om_r, om_b, G));
+    } else
     kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                            static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                            rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
@@ -577,6 +622,91 @@ int step_tma(lb_ctx* c) {
     if (rc != LB_OK) return rc;
     c->cur ^= 1;
     c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
+    c->hx_valid = false;
+    c->diag_fresh = false;
+    return LB_OK;
+}
+
+// ----------------------------------------------------------------------------------------
+// halo kernel (lb_halo.cuh): boxes without solid nodes
+// ----------------------------------------------------------------------------------------
+template <typename T>
+EdgeView<T> edge_view(const lb_ctx* c, int r) {
+    EdgeView<T> v;
+    v.er = static_cast<T*>(c->rho_er[r]); v.ec = static_cast<T*>(c->rho_ec[r]);
+    v.x = static_cast<T*>(c->rho_x[r]); v.s_x = c->s_x;
+    v.y = static_cast<T*>(c->rho_y[r]); v.s_y = c->s_y;
+    v.xy = static_cast<T*>(c->rho_xy[r]); v.s_xy = c->s_xy;
+    return v;
+}
+
+// the frame-density arrays [rcur] and the x-halo copies hx[cur] of the state in f[cur]
+template <typename T>
+int ensure_halo_state(lb_ctx* c) {
+    if (!(c->rho_valid && c->rho_fmt == RHO_EDGE)) {
+        const int r = c->rcur;
+        CU(cudaMemsetAsync(c->rho_x[r], 0, size_t(2) * c->s_x * sizeof(T), c->stream));
+        CU(cudaMemsetAsync(c->rho_y[r], 0, size_t(2) * c->s_y * sizeof(T), c->stream));
+        CU(cudaMemsetAsync(c->rho_xy[r], 0, size_t(2) * c->s_xy * sizeof(T), c->stream));
+        k_density<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), nullptr, c->NP, c->nx, c->ny, c->nz,
+                                                                   static_cast<T*>(c->rho_in[r]));
+        k_edges_from_rho<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->rho_in[r]), c->NP, edge_view<T>(c, r),
+                                                                          c->nx, c->ny, c->nz, OP_TY);
+        c->launches += 2;
+        CU(cudaGetLastError());
+        c->rho_valid = true;
+        c->rho_fmt = RHO_EDGE;
+    }
+    if (!c->hx_valid) {
+        k_fill_xhalo<T><<<blocks_for(c->hx_elems, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), static_cast<T*>(c->hx[c->cur]),
+                                                                             c->NP, c->nx, c->ny, c->nz);
+        c->launches++;
+        CU(cudaGetLastError());
+        c->hx_valid = true;
+    }
+    return LB_OK;
+}
+
+int ensure_diag_buf(lb_ctx* c, long long ncta) {
+    if (c->diag_cta && c->diag_cta_cap >= ncta) return LB_OK;
+    CU(cudaStreamSynchronize(c->stream));
+    cudaFree(c->diag_cta);
+    c->diag_cta = nullptr;
+    CU(cudaMalloc(&c->diag_cta, size_t(ncta) * 5 * sizeof(double)));
+    c->diag_cta_cap = ncta;
+    return LB_OK;
+}
+
+template <typename T, bool DIAG>
+int launch_halo(lb_ctx* c) {
+    auto kern = k_step_halo<T, DIAG, OP_TY>;
+    constexpr size_t smem = HaloLayout<T, OP_TY>::template bytes<DIAG>();
+    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, c->nz / c->zc_tma);
+    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
+    if (DIAG) {
+        const long long ncta = (long long)grid.x * grid.y * grid.z;
+        const int rc = ensure_diag_buf(c, ncta);
+        if (rc != LB_OK) return rc;
+        c->diag_ncta = ncta;
+    }
+    kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap_hx[c->cur], static_cast<const T*>(c->f[c->cur]),
+                                                           static_cast<T*>(c->f[c->cur ^ 1]), static_cast<T*>(c->hx[c->cur ^ 1]),
+                                                           edge_view<T>(c, c->rcur), edge_view<T>(c, c->rcur ^ 1), c->diag_cta,
+                                                           c->NP, c->nx, c->ny, c->nz, c->zc_tma, om_r, om_b, G);
+    c->launches += 1;
+    CU(cudaGetLastError());
+    return LB_OK;
+}
+
+template <typename T>
+int step_halo(lb_ctx* c) {
+    int rc = ensure_halo_state<T>(c);
+    if (rc != LB_OK) return rc;
+    rc = c->diag_mode ? launch_halo<T, true>(c) : launch_halo<T, false>(c);
+    if (rc != LB_OK) return rc;
+    c->cur ^= 1;
+    c->rcur ^= 1;                                           // the kernel wrote the frame densities of t+1 ...
+    c->diag_fresh = c->diag_mode != 0;                      // ... the x-halo copies of the new populations, and (DIAG) their sums
     return LB_OK;
 }
 
@@ -588,6 +718,8 @@ int configure_onepass_kernels() {
     CU(cudaFuncSetAttribute(k_step_pull<T, true, OP_TX, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(onepass_smem_bytes<T, OP_TX, OP_TY>())));
     CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_tma<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
+    CU(cudaFuncSetAttribute(k_step_halo<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<false>())));
+    CU(cudaFuncSetAttribute(k_step_halo<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<true>())));
     return LB_OK;
 }
 
@@ -614,13 +746,16 @@ int tma_zc(const lb_ctx* c) {
     return best;
 }
 
+// LB_KERNEL_HALO has no bounce-back: a box with solid nodes runs the TMA kernel instead (decided per step, effective_kernel)
 int resolve_kernel(lb_ctx* c, int kind) {
     const bool tma_ok = onepass_ok(c) && c->have_tmap;
     if (kind == LB_KERNEL_AUTO) return tma_ok ? LB_KERNEL_TMA : (onepass_ok(c) ? LB_KERNEL_ONEPASS : LB_KERNEL_TWOPASS);
     if (kind == LB_KERNEL_ONEPASS && !onepass_ok(c)) return -1;
-    if (kind == LB_KERNEL_TMA && !tma_ok) return -1;
+    if ((kind == LB_KERNEL_TMA || kind == LB_KERNEL_HALO) && !tma_ok) return -1;
     return kind;
 }
+
+int effective_kernel(const lb_ctx* c) { return c->kernel == LB_KERNEL_HALO && c->has_solid ? LB_KERNEL_TMA : c->kernel; }
 
 long long round64(long long v) { return (v + 63) / 64 * 64; }
 
@@ -682,7 +817,11 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
             ok = ok && cudaMalloc(&c->rho_x[r], size_t(2) * c->s_x * es) == cudaSuccess;
             ok = ok && cudaMalloc(&c->rho_y[r], size_t(2) * c->s_y * es) == cudaSuccess;
             ok = ok && cudaMalloc(&c->rho_xy[r], size_t(2) * c->s_xy * es) == cudaSuccess;
+            ok = ok && cudaMalloc(&c->rho_er[r], size_t(2) * c->s_y * es) == cudaSuccess;
+            ok = ok && cudaMalloc(&c->rho_ec[r], size_t(2) * c->s_x * es) == cudaSuccess;
         }
+        c->hx_elems = (long long)2 * NHALO * nz * ntx * ny;
+        for (int b = 0; b < 2; ++b) ok = ok && cudaMalloc(&c->hx[b], size_t(c->hx_elems) * es) == cudaSuccess;
     }
     ok = ok && cudaMalloc(&c->links, size_t(c->N) * sizeof(unsigned)) == cudaSuccess;
     c->stage_nodes = c->N < STAGE_NODES ? c->N : STAGE_NODES;
@@ -705,6 +844,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
         return nullptr;                                  // LB_ECUDA, message set
     }
     c->have_tmap = onepass_ok(c) && make_tmaps(c);
+    c->cluster_x = 1;
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
     c->zc = onepass_zc(c);
@@ -721,8 +861,11 @@ void lb_destroy(lb_ctx* c) {
     DeviceGuard guard(c->device);
     cudaStreamSynchronize(c->stream);
     cudaFree(c->f[0]); cudaFree(c->f[1]); cudaFree(c->links);
-    for (int r = 0; r < 2; ++r) { cudaFree(c->rho_in[r]); cudaFree(c->rho_x[r]); cudaFree(c->rho_y[r]); cudaFree(c->rho_xy[r]); }
-    cudaFree(c->stage); cudaFree(c->diag_part); cudaFree(c->diag_out);
+    for (int r = 0; r < 2; ++r) {
+        cudaFree(c->rho_in[r]); cudaFree(c->rho_x[r]); cudaFree(c->rho_y[r]); cudaFree(c->rho_xy[r]);
+        cudaFree(c->rho_er[r]); cudaFree(c->rho_ec[r]); cudaFree(c->hx[r]);
+    }
+    cudaFree(c->stage); cudaFree(c->diag_part); cudaFree(c->diag_out); cudaFree(c->diag_cta);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
 }
@@ -736,7 +879,7 @@ int lb_sync(lb_ctx* c) {
 
 long long lb_launch_count(const lb_ctx* c) { return c ? c->launches : 0; }
 
-int lb_get_kernel(const lb_ctx* c) { return c ? c->kernel : -1; }
+int lb_get_kernel(const lb_ctx* c) { return c ? effective_kernel(c) : -1; }
 
 int lb_set_option(lb_ctx* c, int option, long long value) {
     if (!c) return fail(LB_EINVAL, "NULL context");
@@ -748,6 +891,15 @@ int lb_set_option(lb_ctx* c, int option, long long value) {
         c->zc = onepass_zc(c);
         c->zc_tma = tma_zc(c);
         return LB_OK;
+    case LB_OPT_CLUSTER:
+        if (value < 1 || value > 8) return fail(LB_EINVAL, "LB_OPT_CLUSTER: 1..8");
+        c->cluster_x = int(value);
+        return LB_OK;
+    case LB_OPT_DIAG:
+        if (value != 0 && value != 1) return fail(LB_EINVAL, "LB_OPT_DIAG: 0 or 1");
+        c->diag_mode = int(value);
+        c->diag_fresh = false;
+        return LB_OK;
     default:
         return fail(LB_EINVAL, "unknown option");
     }
@@ -756,14 +908,17 @@ int lb_set_option(lb_ctx* c, int option, long long value) {
 long long lb_get_option(const lb_ctx* c, int option) {
     if (!c) return -1;
     switch (option) {
-    case LB_OPT_ZC: return c->kernel == LB_KERNEL_TMA ? c->zc_tma : c->zc;
+    case LB_OPT_ZC: return (c->kernel == LB_KERNEL_TMA || c->kernel == LB_KERNEL_HALO) ? c->zc_tma : c->zc;
+    case LB_OPT_DIAG: return c->diag_mode;
+    case LB_OPT_CLUSTER: return c->cluster_x;
     default: return -1;
     }
 }
 
 int lb_set_kernel(lb_ctx* c, int kind) {
     if (!c) return fail(LB_EINVAL, "NULL context");
-    if (kind != LB_KERNEL_AUTO && kind != LB_KERNEL_TWOPASS && kind != LB_KERNEL_ONEPASS && kind != LB_KERNEL_TMA) return fail(LB_EINVAL, "unknown kernel kind");
+    if (kind != LB_KERNEL_AUTO && kind != LB_KERNEL_TWOPASS && kind != LB_KERNEL_ONEPASS && kind != LB_KERNEL_TMA && kind != LB_KERNEL_HALO)
+        return fail(LB_EINVAL, "unknown kernel kind");
     const int r = resolve_kernel(c, kind);
     if (r < 0) return fail(LB_EINVAL, "box shape does not allow this kernel");
     if (r != c->kernel) c->rho_valid = false;               // the density edge arrays are laid out per tile shape
@@ -878,8 +1033,10 @@ int lb_step(lb_ctx* c, int nsteps) {
     if (!c->have_fields) return fail(LB_ESTATE, "lb_step before lb_set_fields / lb_set_populations");
     for (int s = 0; s < nsteps; ++s) {
         int rc;
-        if (c->kernel == LB_KERNEL_TMA) rc = c->dtype == LB_F64 ? step_tma<double>(c) : step_tma<float>(c);
-        else if (c->kernel == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);
+        const int kern = effective_kernel(c);
+        if (kern == LB_KERNEL_HALO) rc = c->dtype == LB_F64 ? step_halo<double>(c) : step_halo<float>(c);
+        else if (kern == LB_KERNEL_TMA) rc = c->dtype == LB_F64 ? step_tma<double>(c) : step_tma<float>(c);
+        else if (kern == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);
         else rc = c->dtype == LB_F64 ? step_twopass<double>(c) : step_twopass<float>(c);
         if (rc != LB_OK) return rc;
     }
@@ -954,12 +1111,18 @@ int lb_get_diagnostics(lb_ctx* c, double mass[2], double momentum[3]) {
     if (!c || !mass || !momentum) return fail(LB_EINVAL, "NULL argument");
     DeviceGuard guard(c->device);
     const unsigned* lk = c->has_solid ? c->links : nullptr;
+    if (c->diag_mode && c->diag_fresh) {
+        // the last step (halo kernel, LB_OPT_DIAG) left the per-CTA sums of the current state behind: no population pass
+        k_diag_final<<<1, 256, 0, c->stream>>>(c->diag_cta, int(c->diag_ncta), c->diag_out);
+        c->launches += 1;
+    } else {
     if (c->dtype == LB_F64)
         k_diag_partial<double><<<DIAG_BLOCKS, 256, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, c->diag_part);
     else
         k_diag_partial<float><<<DIAG_BLOCKS, 256, 0, c->stream>>>(static_cast<const float*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, c->diag_part);
     k_diag_final<<<1, 256, 0, c->stream>>>(c->diag_part, DIAG_BLOCKS, c->diag_out);
     c->launches += 2;
+    }
     CU(cudaGetLastError());
     double h[5];
     CU(cudaMemcpyAsync(h, c->diag_out, sizeof(h), cudaMemcpyDeviceToHost, c->stream));

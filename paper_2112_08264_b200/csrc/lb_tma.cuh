@@ -64,6 +64,16 @@ __device__ __forceinline__ void mbar_wait2(void* bar_a, void* bar_b, unsigned pa
         "and.pred PA, PA, PB;\n\t"
         "@!PA bra LAB_WAIT2;\n\t}" ::"r"(smem_u32(bar_a)), "r"(smem_u32(bar_b)), "r"(parity) : "memory");
 }
+__device__ __forceinline__ void mbar_wait3(void* bar_a, void* bar_b, void* bar_c, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred PA, PB, PC;\n\tLAB_WAIT3:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 PA, [%0], %3, 0x989680;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 PB, [%1], %3, 0x989680;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 PC, [%2], %3, 0x989680;\n\t"
+        "and.pred PA, PA, PB;\n\t"
+        "and.pred PA, PA, PC;\n\t"
+        "@!PA bra LAB_WAIT3;\n\t}" ::"r"(smem_u32(bar_a)), "r"(smem_u32(bar_b)), "r"(smem_u32(bar_c)), "r"(parity) : "memory");
+}
 // box load: coordinates (x, y, z, plane); x * sizeof(T) must be a multiple of 16 (see header)
 __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int c0, int c1, int c2, int c3) {
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"

@@ -12,8 +12,8 @@ from paper_2112_08264_b200 import workloads as w
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [B.LB_KERNEL_TWOPASS, B.LB_KERNEL_ONEPASS, B.LB_KERNEL_TMA]
-KNAME = {B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass", B.LB_KERNEL_TMA: "tma"}
+KERNELS = [B.LB_KERNEL_TWOPASS, B.LB_KERNEL_ONEPASS, B.LB_KERNEL_TMA, B.LB_KERNEL_HALO]
+KNAME = {B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass", B.LB_KERNEL_TMA: "tma", B.LB_KERNEL_HALO: "halo"}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -288,7 +288,7 @@ def test_full_size_sampled_outputs_and_invariants(oracle_mod, cfg_idx, dtype, to
     rr, rb = cfg.fields()
     R, Bl = rr.reshape(nz, ny, nx), rb.reshape(nz, ny, nx)
     with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype) as box:
-        assert B.lb_kernel_name(box.h) == "tma"
+        assert B.lb_kernel_name(box.h) == "tma"                  # the default kernel, as bench.py times it
         box.set_fields(rr, rb)
         m0, p0 = box.get_diagnostics()
         box.step(s)
@@ -323,9 +323,9 @@ def test_config4_spheres_full_size_sampled_populations(oracle_mod):
     mask = cfg.solid_mask()
     R, Bl, M = rr.reshape(nz, ny, nx), rb.reshape(nz, ny, nx), mask.reshape(nz, ny, nx)
     with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G) as box:
-        assert B.lb_kernel_name(box.h) == "tma"
         box.set_solid_mask(mask)
         box.set_fields(rr, rb)
+        assert B.lb_kernel_name(box.h) == "tma"                  # with solid nodes the default is the TMA kernel (bounce-back)
         zc = box.get_option(B.LB_OPT_ZC)
         links = box.get_link_mask().reshape(nz, ny, nx)
         m0, _ = box.get_diagnostics()
@@ -381,7 +381,7 @@ def test_headline_512_cube_sampled_moments_and_invariants(oracle_mod, cfg_idx, d
     rr, rb = cfg.fields()
     R, Bl = rr.reshape(nz, ny, nx), rb.reshape(nz, ny, nx)
     with B.Box(nx, ny, nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype) as box:
-        assert B.lb_kernel_name(box.h) == "tma"
+        assert B.lb_kernel_name(box.h) == "tma"                  # the default kernel, as bench.py times it
         box.set_fields(rr, rb)
         m0, p0 = box.get_diagnostics()
         box.step(s)
@@ -426,6 +426,37 @@ def test_state_and_argument_errors():
             box.set_kernel(99)
         box.step(0)
         assert box.launch_count() > 0
+
+
+@pytest.mark.parametrize("dtype,tol_m,tol_p", [(B.LB_F64, 1e-13, 1e-10), (B.LB_F32, 1e-5, 1e-3)])
+def test_fused_per_step_diagnostics_match_oracle(oracle_mod, dtype, tol_m, tol_p):
+    """LB_OPT_DIAG: the halo step kernel leaves the mass / momentum sums of the NEW state behind (warp shuffles -> per-CTA
+    partial -> fixed-order final); lb_get_diagnostics then makes no population pass.  Every one of config 0's 100 steps
+    against the oracle's compensated sums (Eq. 6-7), and against the separate-pass diagnostics of the same state."""
+    cfg = w.CONFIGS[0]
+    rr, rb = cfg.fields()
+    o = oracle_mod.Oracle(cfg.nx, cfg.ny, cfg.nz, 0.8, 1.3, 0.9)
+    o.set_fields(rr, rb)
+    with B.Box(cfg.nx, cfg.ny, cfg.nz, 0.8, 1.3, 0.9, dtype=dtype) as box:
+        box.set_kernel(B.LB_KERNEL_HALO)
+        box.set_option(B.LB_OPT_DIAG, 1)
+        box.set_fields(rr, rb)
+        worst_m = worst_p = 0.0
+        for t in range(100):
+            o.step(1), box.step(1)
+            l0 = box.launch_count()
+            gm, gp = box.get_diagnostics()
+            assert box.launch_count() - l0 == 1                  # k_diag_final only: no pass over the populations
+            om, op = o.get_diagnostics()
+            worst_m = max(worst_m, float(np.abs(gm / om - 1).max()))
+            worst_p = max(worst_p, float(np.abs(gp - op).max()))
+            if t in (0, 49, 99):
+                box.set_option(B.LB_OPT_DIAG, 0)                 # the separate pass over the same state
+                sm_, sp_ = box.get_diagnostics()
+                box.set_option(B.LB_OPT_DIAG, 1)
+                assert np.abs(gm / sm_ - 1).max() < tol_m and np.abs(gp - sp_).max() < tol_p
+        print(f"fused diagnostics dtype {dtype}: worst mass rel err {worst_m:.3e}, momentum abs err {worst_p:.3e}")
+        assert worst_m < tol_m and worst_p < tol_p
 
 
 def test_diagnostics_are_deterministic_and_match_fields():
