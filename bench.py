@@ -182,7 +182,7 @@ def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return 0
-    cfg = with_overrides(WORKLOADS["config2" if args.workload == "all" else args.workload], args)
+    cfg = with_overrides(WORKLOADS["config2" if args.workload == "all" or args.workload in SINGLE else args.workload], args)
     sub = (min(cfg.nx, 64), min(cfg.ny, 32), min(cfg.nz, 32))
     glups, dt = time_oracle(cfg, sub, args.steps, args.warmup)
     sample = (f"periodic {sub[0]}x{sub[1]}x{sub[2]} corner of {cfg.name}'s seeded fields, "
@@ -222,12 +222,75 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     B.lib()
-    names = sorted(WORKLOADS) if args.workload == "all" else [args.workload]
+    names = sorted(WORKLOADS) + sorted(SINGLE) if args.workload == "all" else [args.workload]
     for i, name in enumerate(names):
+        if name in SINGLE:
+            run_single(args, name, B, torch, dev, rank, local_rank, world)
+            continue
         # `all`: the CPU oracle is timed once (on the headline workload), not five times
         cpu = not args.no_cpu_baseline and (args.workload != "all" or name == "config2")
         run_one(args, with_overrides(WORKLOADS[name], args), B, torch, dev, rank, local_rank, world, cpu)
     return 0
+
+
+SINGLE = {"single128_f32": (128, "f32"), "single256_f32": (256, "f32"), "single256_f64": (256, "f64"), "single512_f32": (512, "f32")}
+
+
+def run_single(args, name, B, torch, dev, rank, local_rank, world):
+    """The single-fluid calibration workload (the paper's case 1, Table 1):
+    one BGK fluid, fused collide + stream, 304 / 152 algorithmic bytes per node.  rho = 1 + 1 % seeded noise, u = 0."""
+    n, dt = SINGLE[name]
+    N = n * n * n
+    tau = args.tau_r if args.tau_r is not None else 1.0
+    steps, warmup = args.steps, max(args.warmup, 3)
+    rho, _ = W.mixture_fields(n, n, n, 2112082645)
+    pin = torch.empty(N, dtype=torch.float64).pin_memory()
+    pin.numpy()[:] = rho
+    out = torch.empty(N, dtype=torch.float64).pin_memory()
+    stream = torch.cuda.Stream(device=dev)
+    box = B.SingleBox(n, n, n, tau, dtype=B.LB_F64 if dt == "f64" else B.LB_F32, cuda_stream=stream.cuda_stream)
+    box.set_fields(pin.numpy())
+    box.step(warmup)
+    box.sync()
+    torch.cuda.synchronize(dev)
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = box.launch_count()
+    e0.record(stream)
+    box.step(steps)
+    e1.record(stream)
+    e1.synchronize()
+    launches = box.launch_count() - l0
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    ms_max, units = aggregate_over_ranks(ms, float(N) * steps, world, dev)
+    glups = units / (ms_max * 1e-3) / 1e9
+    t0 = time.perf_counter()
+    box.set_fields(pin.numpy())
+    box.step(steps)
+    B._chk(B.lib().lbs_get_moments(box.h, B._d(out.numpy()), None, None, None))
+    e2e_s = time.perf_counter() - t0
+    box.close()
+    if rank != 0:
+        return
+    peak, peak_src = measured_peak()
+    alg = ALG_BYTES[dt] // 2
+    achieved = alg * N / (ms / steps * 1e-3) / 1e9
+    es = 8 if dt == "f64" else 4
+    line = {
+        "metric": "GLUPS (single-fluid D3Q19 BGK, fused collide + stream) on 1 B200; achieved HBM GB/s vs peak", "value": glups, "unit": "GLUPS",
+        "n_gpus": world, "steps": steps, "warmup": warmup, "ms_per_step": ms_max / steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": dt, "data": "synthetic",
+        "config": {"workload": name, "box": [n, n, n], "tau": [tau], "kernel": "single", "launches_per_step": launches / steps,
+                   "l2": f"state {2 * 19 * N * es / 2**30:.1f} GiB vs 126 MB L2",
+                   "context": "paper Table 1 (PAPER.md:175-194): 2.011 GLUPS fused at 256^3 fp32 on 1 V100; 3.406 quoted as state of the art (PAPER.md:192)"},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_node": alg, "kernel_ms": ms / steps, "kernel": "k_single_step"},
+        "e2e": {"value": N * steps / e2e_s / 1e9, "unit": "GLUPS", "h2d_bytes_per_step": N * 8 / steps, "d2h_bytes_per_step": N * 8 / steps,
+                "seconds": e2e_s, "calls": "lbs_set_fields(host) + lbs_step(K) + lbs_get_moments(host rho)"},
+        "gpu_launches": launches, "clocks": clocks,
+    }
+    print(json.dumps(line), flush=True)
 
 
 def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
@@ -356,7 +419,7 @@ def main():
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS) + ["all"])
+    ap.add_argument("--workload", default="config2", choices=sorted(WORKLOADS) + sorted(SINGLE) + ["all"])
     ap.add_argument("--tau-r", type=float, default=None, help="override the workload's tau_r (general-tau variant)")
     ap.add_argument("--tau-b", type=float, default=None)
     ap.add_argument("--G", type=float, default=None)

@@ -119,17 +119,29 @@ int lb_get_diagnostics(lb_ctx* ctx, double mass[2], double momentum[3]);
  * (reads the populations twice per step); LB_KERNEL_ONEPASS = single fused pass that
  * reads and writes every population once per step, populations pulled with per-thread loads;
  * LB_KERNEL_TMA = the same single pass with the populations staged in shared memory by the TMA
- * unit (the fastest; needs nx % 32 == 0 and ny % 8 == 0 like ONEPASS); LB_KERNEL_AUTO (default) =
- * TMA when the box shape allows it (ONEPASS if the driver cannot encode the tensor maps), else
+ * unit (the fastest; needs nx % 32 == 0 and ny % 8 == 0 like ONEPASS); LB_KERNEL_HALO = a second
+ * TMA-staged single pass that reads aligned tiles only (the x neighbour's column comes from
+ * x-halo copies) and sums the density of the tile's own nodes from the staged populations
+ * instead of carrying it (less DRAM traffic, measured slower; no bounce-back: a box with solid
+ * nodes runs LB_KERNEL_TMA instead; the only kernel with LB_OPT_DIAG); LB_KERNEL_AUTO (default)
+ * = TMA when the box shape allows it (ONEPASS if the driver cannot encode the tensor maps), else
  * TWOPASS: boxes whose sides are not multiples of the 32 x 8 tile run about 1.5 x slower.
  * LB_EINVAL if the box shape does not allow `kind`. */
 int lb_set_kernel(lb_ctx* ctx, int kind);
 
-/* The kernel lb_step will use (LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS or LB_KERNEL_TMA; never AUTO); -1 for a NULL context. */
+/* The kernel lb_step will use (LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA or LB_KERNEL_HALO; never AUTO); -1 for a NULL context. */
 int lb_get_kernel(const lb_ctx* ctx);
 
 /* Tuning and modes.  LB_OPT_ZC: planes per CTA of the one-pass kernels (each CTA marches over
  * value z planes and re-collides one more at either end); 0 = the library's heuristic (default).
+ * LB_OPT_DIAG (0 / 1, default 0): per-step diagnostics fused into the step: with LB_KERNEL_HALO
+ * every lb_step leaves the per-component mass and the total momentum of the NEW state behind
+ * (per thread in shared memory, warp shuffles, one partial per CTA, added in a fixed order), and
+ * lb_get_diagnostics then makes no pass over the populations; the momentum is the sum of the
+ * post-collision moments (1 - omega_k) j^k + omega_k rho^k u' + rho^k du^k, which streaming in a
+ * periodic box only permutes.  With any other kernel the option changes nothing.
+ * LB_OPT_CLUSTER (1..8, default 1): launch LB_KERNEL_TMA in thread-block clusters of that many
+ * x-adjacent tiles (measured: no gain).
  * LB_EINVAL for an unknown option or a value out of range.  lb_get_option returns the value in
  * effect (for LB_OPT_ZC: the planes per CTA the current kernel will use), -1 on error. */
 int lb_set_option(lb_ctx* ctx, int option, long long value);
@@ -150,6 +162,24 @@ int lb_last_error_code(void);
 
 /* Library version string. */
 const char* lb_version(void);
+
+/* ---- single-fluid calibration path (the paper's case 1, Table 1) --------------
+ * One BGK fluid on the same D3Q19 lattice, periodic box, no force, no solids, fused collide +
+ * stream: f_i(x + c_i, t + 1) = (1 - omega) f_i + omega feq_i(rho, u) (Eq. 1, PAPER.md:77-80;
+ * Eq. 10), 19 * 2 values moved per node and step (304 B in fp64, 152 B in fp32:
+ * the paper's B = 19 x 2 x 8 per fluid).  Same conventions as above (host
+ * pointers, dense [z][y][x] arrays, doubles at the boundary, error codes, lb_last_error).
+ * Any box shape with ny, nz <= 65535.  Populations: 19 * N doubles, [i][z][y][x]. */
+typedef struct lbs_ctx lbs_ctx;
+lbs_ctx* lbs_create(int nx, int ny, int nz, double tau, int dtype, void* cuda_stream);   /* NULL on failure */
+void lbs_destroy(lbs_ctx* ctx);
+int  lbs_set_fields(lbs_ctx* ctx, const double* rho, const double* ux, const double* uy, const double* uz);   /* u: all NULL = 0 */
+int  lbs_set_populations(lbs_ctx* ctx, const double* f);
+int  lbs_step(lbs_ctx* ctx, int nsteps);                       /* asynchronous; LB_ESTATE before a set call */
+int  lbs_get_populations(lbs_ctx* ctx, double* f);             /* synchronises */
+int  lbs_get_moments(lbs_ctx* ctx, double* rho, double* ux, double* uy, double* uz);   /* any pointer may be NULL */
+int  lbs_sync(lbs_ctx* ctx);
+long long lbs_launch_count(const lbs_ctx* ctx);
 
 #ifdef __cplusplus
 }

@@ -28,6 +28,8 @@ SYMBOLS = (
     "lb_set_populations", "lb_step", "lb_get_populations", "lb_get_moments",
     "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
     "lb_set_option", "lb_get_option", "lb_sync", "lb_last_error", "lb_last_error_code", "lb_version",
+    "lbs_create", "lbs_destroy", "lbs_set_fields", "lbs_set_populations", "lbs_step", "lbs_get_populations",
+    "lbs_get_moments", "lbs_sync", "lbs_launch_count",
 )
 
 _dp = C.POINTER(C.c_double)
@@ -74,6 +76,18 @@ def lib() -> C.CDLL:
     L.lb_sync.argtypes = [C.c_void_p]
     L.lb_last_error.restype = C.c_char_p
     L.lb_version.restype = C.c_char_p
+    L.lbs_create.restype = C.c_void_p
+    L.lbs_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p]
+    L.lbs_destroy.restype = None
+    L.lbs_destroy.argtypes = [C.c_void_p]
+    L.lbs_set_fields.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
+    L.lbs_set_populations.argtypes = [C.c_void_p, _dp]
+    L.lbs_step.argtypes = [C.c_void_p, C.c_int]
+    L.lbs_get_populations.argtypes = [C.c_void_p, _dp]
+    L.lbs_get_moments.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp]
+    L.lbs_sync.argtypes = [C.c_void_p]
+    L.lbs_launch_count.restype = C.c_longlong
+    L.lbs_launch_count.argtypes = [C.c_void_p]
     _lib = L
     return L
 
@@ -258,3 +272,53 @@ class Box:
 
     def sync(self):
         lb_sync(self.h)
+
+
+class SingleBox:
+    """Convenience owner of one lbs_ctx: the single-fluid calibration path (lbs_* calls)."""
+
+    def __init__(self, nx, ny, nz, tau=1.0, dtype=LB_F64, cuda_stream=None):
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.N = nx * ny * nz
+        self.h = lib().lbs_create(nx, ny, nz, tau, dtype, cuda_stream)
+        if not self.h:
+            raise LBError(lb_last_error_code(), lb_last_error())
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().lbs_destroy(self.h)
+            self.h = None
+
+    __del__ = close
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def set_fields(self, rho, ux=None, uy=None, uz=None):
+        a = [_host_f64(v, self.N, nm) for v, nm in zip((rho, ux, uy, uz), ("rho", "ux", "uy", "uz"))]
+        _chk(lib().lbs_set_fields(self.h, *[_d(v) for v in a]))
+
+    def set_populations(self, f):
+        _chk(lib().lbs_set_populations(self.h, _d(_host_f64(f, 19 * self.N, "f"))))
+
+    def step(self, nsteps=1):
+        _chk(lib().lbs_step(self.h, nsteps))
+
+    def get_populations(self):
+        f = np.empty(19 * self.N, dtype=np.float64)
+        _chk(lib().lbs_get_populations(self.h, _d(f)))
+        return f.reshape(19, self.nz, self.ny, self.nx)
+
+    def get_moments(self):
+        o = [np.empty(self.N, dtype=np.float64) for _ in range(4)]
+        _chk(lib().lbs_get_moments(self.h, *[_d(v) for v in o]))
+        return o
+
+    def sync(self):
+        _chk(lib().lbs_sync(self.h))
+
+    def launch_count(self):
+        return int(lib().lbs_launch_count(self.h))

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB_DIR = os.path.join(_HERE, "_lib")
 LIB_PATH = os.path.join(LIB_DIR, "liblb_b200.so")
-SOURCES = [os.path.join(CSRC, "lb_b200.cu")]
+SOURCES = [os.path.join(CSRC, "lb_b200.cu"), os.path.join(CSRC, "lb_single.cu")]
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
     "-Xcompiler", "-fPIC", "-shared", "--fmad=true",

@@ -761,6 +761,9 @@ long long round64(long long v) { return (v + 63) / 64 * 64; }
 
 }  // namespace
 
+// the library's error slot (one per thread), shared with lb_single.cu
+void lb_set_error(int code, const char* what) { g_err = what; g_err_code = code; }
+
 // ----------------------------------------------------------------------------------------
 // C ABI
 // ----------------------------------------------------------------------------------------

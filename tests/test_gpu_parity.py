@@ -407,6 +407,55 @@ def test_headline_512_cube_sampled_moments_and_invariants(oracle_mod, cfg_idx, d
 
 
 # ---------------------------------------------------------------------------------------------
+# single-fluid calibration path (lbs_*): the oracle with rho_b = 0 is the single-fluid BGK (pin P5-single)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype,tol", [(B.LB_F64, 1e-13), (B.LB_F32, 5e-6)])
+@pytest.mark.parametrize("shape,tau", [((32, 32, 32), 1.0), ((40, 24, 12), 0.8), ((130, 5, 3), 0.6), ((1, 1, 1), 0.9), ((2, 3, 5), 1.3)])
+def test_single_fluid_against_oracle(oracle_mod, dtype, tol, shape, tau):
+    nx, ny, nz = shape
+    N = nx * ny * nz
+    rng = np.random.default_rng(17)
+    rho = 1.0 + 0.01 * rng.uniform(-1, 1, N)
+    u = rng.uniform(-0.03, 0.03, (3, N))
+    o = oracle_mod.Oracle(nx, ny, nz, tau, 1.0, 1.2)
+    o.set_fields(rho, np.zeros(N), *u)
+    with B.SingleBox(nx, ny, nz, tau, dtype=dtype) as box:
+        box.set_fields(rho, *u)
+        assert nerr(box.get_populations(), o.get_populations()[0]) < (1e-15 if dtype == B.LB_F64 else 1e-6)
+        for steps in (1, 9, 40):
+            o.step(steps), box.step(steps)
+            e = nerr(box.get_populations(), o.get_populations()[0])
+            assert e < tol, (steps, e)
+        gm, om = box.get_moments(), o.get_moments()
+        assert np.abs(gm[0] - om[0]).max() < 10 * tol
+        for a in range(3):
+            assert np.abs(gm[1 + a] - om[2 + a]).max() < 10 * tol
+        assert box.launch_count() > 0
+
+
+def test_single_fluid_random_populations_and_errors(oracle_mod):
+    nx, ny, nz = 64, 8, 4
+    N = nx * ny * nz
+    rng = np.random.default_rng(2)
+    f0 = rng.uniform(0.01, 0.1, 19 * N)                          # non-equilibrium
+    f2 = np.concatenate([f0, np.zeros(19 * N)])
+    o = oracle_mod.Oracle(nx, ny, nz, 0.7, 1.0, 0.0)
+    o.set_populations(f2)
+    with B.SingleBox(nx, ny, nz, 0.7) as box:
+        with pytest.raises(B.LBError) as ei:
+            box.step(1)
+        assert ei.value.code == B.LB_ESTATE
+        box.set_populations(f0)
+        assert np.array_equal(box.get_populations().reshape(-1), f0)   # set -> get is a pure move
+        for _ in range(3):
+            o.step(1), box.step(1)
+            assert nerr(box.get_populations(), o.get_populations()[0]) < 1e-14
+    with pytest.raises(B.LBError) as ei:
+        B.SingleBox(4, 4, 4, 0.5)
+    assert ei.value.code == B.LB_EINVAL
+
+
+# ---------------------------------------------------------------------------------------------
 # API behaviour on the device
 # ---------------------------------------------------------------------------------------------
 def test_state_and_argument_errors():

@@ -146,6 +146,28 @@ def test_p5_shear_wave_decay(oracle_mod, tau, tol):
     assert abs(rate / (nu * k2) - 1) < tol
 
 
+def test_p5_single_fluid_reduction(oracle_mod):
+    """rho_b = 0 turns the two-component update into the plain single-fluid BGK of Eq. 1 (reading S6: no division by
+    rho^k; the empty component exerts no force and stays exactly empty), for any G.  Pinned by the same shear wave:
+    nu = c_s^2 (tau - 1/2), Eq. 2 PAPER.md:84.  This is the oracle of the single-fluid calibration path (lbs_*)."""
+    nx, ny, nz, U, steps, tau = 4, 32, 4, 1e-3, 200, 0.8
+    y = np.arange(ny)
+    ux = np.broadcast_to((U * np.sin(2 * np.pi * y / ny))[None, :, None], (nz, ny, nx)).reshape(-1).copy()
+    o = oracle_mod.Oracle(nx, ny, nz, tau, 1.7, 1.2)            # the blue relaxation time and G must not matter
+    o.set_fields(np.ones(nx * ny * nz), np.zeros(nx * ny * nz), ux, None, None)
+    amp = []
+    for _ in range(steps + 1):
+        u = o.get_moments()[2].reshape(nz, ny, nx)
+        amp.append(2.0 / ny * (u[0, :, 0] * np.sin(2 * np.pi * y / ny)).sum())
+        o.step(1)
+    f = o.get_populations()
+    assert np.all(f[1] == 0.0)                                   # the empty component stays exactly empty
+    assert np.all(np.isfinite(f[0]))
+    k2 = (2 * np.pi / ny) ** 2
+    rate = -np.polyfit(np.arange(100, steps + 1), np.log(np.array(amp)[100:]), 1)[0]
+    assert abs(rate / ((tau - 0.5) / 3.0 * k2) - 1) < 0.02
+
+
 # P6 ------------------------------------------------------------------------
 def test_p6_force_on_sine_profile(oracle_mod):
     nx, ny, nz, G, a, b = 32, 3, 5, 1.2, 1.0, 0.2
