@@ -78,6 +78,13 @@ def _load(variant: str) -> C.CDLL:
     lib.ora_feq.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, _dp]
     lib.ora_lattice.restype = None
     lib.ora_lattice.argtypes = [C.POINTER(C.c_int), _dp]
+    lib.ora_set_colour_gradient.argtypes = [C.c_void_p, C.c_double, C.c_double]
+    lib.ora_get_phase_field.argtypes = [C.c_void_p, _dp, _dp]
+    lib.ora_cg_perturbation.restype = None
+    lib.ora_cg_perturbation.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, _dp]
+    lib.ora_set_spheres.argtypes = [C.c_void_p, C.c_int, _dp, C.c_double, _dp, _dp]
+    lib.ora_get_sphere_forces.argtypes = [C.c_void_p, _dp, _dp]
+    lib.ora_get_solid_mask.argtypes = [C.c_void_p, C.POINTER(C.c_ubyte)]
     _libs[variant] = lib
     return lib
 
@@ -98,6 +105,12 @@ def _f64(a, n):
 def feq(rho, ux, uy, uz, variant: str = "ref"):
     out = np.empty(19)
     _load(variant).ora_feq(rho, ux, uy, uz, _d(out))
+    return out
+
+
+def cg_perturbation(A, gx, gy, gz, variant: str = "ref"):
+    out = np.empty(19)
+    _load(variant).ora_cg_perturbation(A, gx, gy, gz, _d(out))
     return out
 
 
@@ -129,6 +142,31 @@ class Oracle:
     def _chk(self, rc):
         if rc != 0:
             raise RuntimeError(f"oracle call failed with code {rc}")
+
+    def set_colour_gradient(self, sigma, beta):
+        self._chk(self._lib.ora_set_colour_gradient(self._h, sigma, beta))
+
+    def get_phase_field(self):
+        th, g = np.empty(self.N), np.empty(3 * self.N)
+        self._chk(self._lib.ora_get_phase_field(self._h, _d(th), _d(g)))
+        return th, g.reshape(3, self.N)
+
+    def set_spheres(self, centres, radius, vel=None, omega=None):
+        c = np.ascontiguousarray(centres, dtype=np.float64).reshape(-1, 3)
+        self.nsph = c.shape[0]
+        v = None if vel is None else _f64(vel, 3 * self.nsph)
+        w = None if omega is None else _f64(omega, 3 * self.nsph)
+        self._chk(self._lib.ora_set_spheres(self._h, self.nsph, _d(c.reshape(-1)), radius, _d(v), _d(w)))
+
+    def get_sphere_forces(self):
+        F, T = np.empty(3 * self.nsph), np.empty(3 * self.nsph)
+        self._chk(self._lib.ora_get_sphere_forces(self._h, _d(F), _d(T)))
+        return F.reshape(-1, 3), T.reshape(-1, 3)
+
+    def get_solid_mask(self):
+        m = np.empty(self.N, dtype=np.uint8)
+        self._chk(self._lib.ora_get_solid_mask(self._h, m.ctypes.data_as(C.POINTER(C.c_ubyte))))
+        return m
 
     def set_forcing(self, mode):
         self._chk(self._lib.ora_set_forcing(self._h, mode))
