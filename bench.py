@@ -140,6 +140,9 @@ def with_overrides(cfg, args):
     """The workload with --tau-r / --tau-b / --G replaced (the general-tau bench variants of SURVEY 8(d) 'rules')."""
     import dataclasses
     kw = {}
+    if getattr(args, "f32", False) and cfg.dtype != "f32":
+        kw["dtype"] = "f32"
+        kw["name"] = cfg.name.replace("f64", "f32")
     if args.tau_r is not None:
         kw["tau_r"] = args.tau_r
     if args.tau_b is not None:
@@ -322,7 +325,14 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
     box.set_kernel(kernel)
     if args.diag:
         box.set_option(B.LB_OPT_DIAG, 1)
-    if mask is not None:
+    if args.model == "cg":                       # the paper's own two-fluid operator, general two-pass path
+        box.set_colour_gradient(args.sigma, args.beta)
+    if mask is not None and args.moving_walls:   # prescribed sphere velocities + force / torque per sphere (N2), same path
+        centres, _ = W.sphere_centres(cfg.nx, cfg.ny, cfg.nz, cfg.sphere_seed, cfg.n_spheres)
+        vel = 0.01 * (2.0 * W.u01(cfg.sphere_seed + 1, np.arange(3 * cfg.n_spheres)) - 1.0)
+        omg = 0.002 * (2.0 * W.u01(cfg.sphere_seed + 2, np.arange(3 * cfg.n_spheres)) - 1.0)
+        box.set_spheres(centres, 5.5, vel, omg)
+    elif mask is not None:
         box.set_solid_mask(mask)
     box.set_fields(rr, rb)
     kname = B.lb_kernel_name(box.h)
@@ -384,6 +394,8 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
                    "solid_spheres": cfg.n_spheres, "kernel": kname, "launches_per_step": launches / steps,
                    "l2": f"state {2 * 38 * N * es / 2**30:.1f} GiB vs 126 MB L2" + (", no flush needed" if 2 * 38 * N * es > (1 << 30) else ": L2-resident, launch-bound, reported only"),
                    "parallelism": "replicas only" if world > 1 else "single GPU", "diagnostics_in_step": bool(args.diag),
+                   "operator": "colour gradient (sigma %g, beta %g)" % (args.sigma, args.beta) if args.model == "cg" else "Shan-Chen",
+                   "moving_walls": bool(mask is not None and args.moving_walls),
                    **({"note": note} if note else {})},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
@@ -423,6 +435,11 @@ def main():
     ap.add_argument("--tau-r", type=float, default=None, help="override the workload's tau_r (general-tau variant)")
     ap.add_argument("--tau-b", type=float, default=None)
     ap.add_argument("--G", type=float, default=None)
+    ap.add_argument("--model", default="sc", choices=["sc", "cg"], help="collision operator: Shan-Chen (north_star) or colour gradient (PAPER.md:328-400)")
+    ap.add_argument("--sigma", type=float, default=0.02)
+    ap.add_argument("--beta", type=float, default=0.7)
+    ap.add_argument("--moving-walls", action="store_true", help="config4: spheres with seeded velocities, force / torque per sphere each step")
+    ap.add_argument("--f32", action="store_true", help="run the workload in fp32 (e.g. config1 --f32 --model cg: the paper's Table 2 setting)")
     ap.add_argument("--diag", action="store_true", help="per-step mass / momentum sums fused into the step kernel (LB_OPT_DIAG)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma", "halo"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

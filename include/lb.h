@@ -45,7 +45,8 @@ typedef struct lb_ctx lb_ctx;          /* opaque; owned by the library */
 enum { LB_OK = 0, LB_EINVAL = -1, LB_ENOMEM = -2, LB_ECUDA = -3, LB_ESTATE = -4 };
 enum { LB_F64 = 0, LB_F32 = 1 };
 enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2, LB_KERNEL_TMA = 3, LB_KERNEL_HALO = 4 };
-enum { LB_OPT_ZC = 1, LB_OPT_DIAG = 2, LB_OPT_CLUSTER = 3 };   /* options of lb_set_option */
+enum { LB_OPT_ZC = 1, LB_OPT_DIAG = 2, LB_OPT_CLUSTER = 3 };
+enum { LB_MODEL_SHAN_CHEN = 0, LB_MODEL_COLOUR_GRADIENT = 1 };   /* options of lb_set_option */
 
 /* Create a context for an nx*ny*nz periodic box holding two fluids with BGK
  * relaxation times tau_r, tau_b (Eq. 1; omega_k = 1/tau_k) coupled by the
@@ -162,6 +163,31 @@ int lb_last_error_code(void);
 
 /* Library version string. */
 const char* lb_version(void);
+
+/* ---- later operators (the paper's own two-fluid model and its moving walls), on the general two-pass path ----------
+ * Colour-gradient collision (Eq. 8-21): replaces the Shan-Chen force + BGK of lb_step by
+ *   Theta = (rho^1 - rho^2) / (rho^1 + rho^2), grad Theta = (1 / c_s^2) sum_i w_i Theta(x + c_i) c_i,
+ *   omega = 2 / (6 nu + 1) with 1 / nu = (rho^1 / rho) / nu_1 + (rho^2 / rho) / nu_2, nu_k = c_s^2 (tau_k - 1/2),
+ *   BGK with that omega towards feq_i(rho^k, u) (Eq. 9-10, u by Eq. 7), the perturbation of Eq. 17 with A = (9/4) sigma omega
+ *   (Eq. 19) and the B_i of PAPER.md:393-398, and the recolouring of Eq. 20-21 with strength beta in [0, 1];
+ * readings C1-C6 of DESIGN.md section 3 for what the paper leaves open or prints garbled.  G is ignored.  Streaming,
+ * bounce-back, fields, getters and diagnostics are unchanged.  lb_set_shan_chen switches back.  LB_EINVAL for a
+ * non-finite sigma or beta outside [0, 1]. */
+int lb_set_colour_gradient(lb_ctx* ctx, double sigma, double beta);
+int lb_set_shan_chen(lb_ctx* ctx);
+
+/* Solid spheres with prescribed velocities (Eq. 22-27): np spheres of one radius, centres[np][3]
+ * real-valued, vel[np][3] and omega[np][3] their translational and angular velocities (NULL = 0).  Sets the solid mask
+ * (a node is solid iff its minimum-image squared distance to a centre <= radius^2, reading S9) like lb_set_solid_mask;
+ * the geometry stays where it is, only the walls move: a link i from fluid node r into sphere p returns
+ *   f_opp(i)^k(r, t+1) = f*_i^k(r) - 2 rho^k(r) w_i (u_b . c_i) / c_s^2,  u_b = v_p + r_b x omega_p,  r_b = r + c_i / 2 - centre_p
+ * (Eq. 22, Eq. 24), and hands F_i = c_i [f*_i + f_opp(i)(t+1)] (both components) to the sphere (Eq. 25-26), with torque
+ * F_i x r_b (Eq. 27); readings M1-M4 of DESIGN.md section 3.  lb_get_sphere_forces returns F[np][3], T[np][3] of the LAST
+ * step, accumulated in fp64 for both dtypes with atomic adds (fp64 accumulators; the order of the sum is
+ * not fixed, as the paper notes for its own GPU code at PAPER.md:240).  np = 0 removes the spheres and all solids;
+ * lb_set_solid_mask afterwards also makes every solid a wall at rest again.  Synchronises. */
+int lb_set_spheres(lb_ctx* ctx, int np, const double* centres, double radius, const double* vel, const double* omega);
+int lb_get_sphere_forces(lb_ctx* ctx, double* F, double* T);
 
 /* ---- single-fluid calibration path (the paper's case 1, Table 1) --------------
  * One BGK fluid on the same D3Q19 lattice, periodic box, no force, no solids, fused collide +

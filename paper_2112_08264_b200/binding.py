@@ -28,6 +28,7 @@ SYMBOLS = (
     "lb_set_populations", "lb_step", "lb_get_populations", "lb_get_moments",
     "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
     "lb_set_option", "lb_get_option", "lb_sync", "lb_last_error", "lb_last_error_code", "lb_version",
+    "lb_set_colour_gradient", "lb_set_shan_chen", "lb_set_spheres", "lb_get_sphere_forces",
     "lbs_create", "lbs_destroy", "lbs_set_fields", "lbs_set_populations", "lbs_step", "lbs_get_populations",
     "lbs_get_moments", "lbs_sync", "lbs_launch_count",
 )
@@ -76,6 +77,10 @@ def lib() -> C.CDLL:
     L.lb_sync.argtypes = [C.c_void_p]
     L.lb_last_error.restype = C.c_char_p
     L.lb_version.restype = C.c_char_p
+    L.lb_set_colour_gradient.argtypes = [C.c_void_p, C.c_double, C.c_double]
+    L.lb_set_shan_chen.argtypes = [C.c_void_p]
+    L.lb_set_spheres.argtypes = [C.c_void_p, C.c_int, _dp, C.c_double, _dp, _dp]
+    L.lb_get_sphere_forces.argtypes = [C.c_void_p, _dp, _dp]
     L.lbs_create.restype = C.c_void_p
     L.lbs_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p]
     L.lbs_destroy.restype = None
@@ -260,6 +265,24 @@ class Box:
 
     def set_kernel(self, kind):
         lb_set_kernel(self.h, kind)
+
+    def set_colour_gradient(self, sigma, beta):
+        _chk(lib().lb_set_colour_gradient(self.h, sigma, beta))
+
+    def set_shan_chen(self):
+        _chk(lib().lb_set_shan_chen(self.h))
+
+    def set_spheres(self, centres, radius, vel=None, omega=None):
+        c = np.ascontiguousarray(centres, dtype=np.float64).reshape(-1, 3)
+        self.nsph = c.shape[0]
+        v = None if vel is None else _host_f64(vel, 3 * self.nsph, "vel")
+        w = None if omega is None else _host_f64(omega, 3 * self.nsph, "omega")
+        _chk(lib().lb_set_spheres(self.h, self.nsph, _d(c.reshape(-1)), radius, _d(v), _d(w)))
+
+    def get_sphere_forces(self):
+        F, T = np.zeros(3 * self.nsph), np.zeros(3 * self.nsph)
+        _chk(lib().lb_get_sphere_forces(self.h, _d(F), _d(T)))
+        return F.reshape(-1, 3), T.reshape(-1, 3)
 
     def set_option(self, option, value):
         lb_set_option(self.h, option, value)

@@ -60,6 +60,14 @@ struct lb_ctx {
     int zc;            // planes per CTA of the one-pass kernel
     int zc_tma;        // ... of the TMA kernel
     CUtensorMap tmap_hx[2];   // [buffer] x-halo box TY x 1 x 1 x 2 over hx [plane][z][tile_x][y]
+    // later operators, both on the general two-pass path
+    int model;         // LB_MODEL_SHAN_CHEN or LB_MODEL_COLOUR_GRADIENT
+    double sigma, beta;
+    bool in_set_spheres;
+    int nsph;          // spheres with prescribed velocities (moving-wall bounce-back, force / torque per sphere)
+    double radius;
+    double* sph;       // device: centres[nsph][3], vel[nsph][3], omega[nsph][3], F[nsph][3], T[nsph][3]
+    int* pid;          // device: sphere of every solid node (-1 = none)
     int cluster_x;     // LB_OPT_CLUSTER: thread-block cluster size along x for the TMA kernel (1 = none)
     int diag_mode;     // LB_OPT_DIAG: the halo kernel also leaves the mass / momentum sums of the new state behind
     bool diag_fresh;   // diag_cta holds the per-CTA partials of the state in f[cur]
@@ -412,6 +420,160 @@ __global__ void __launch_bounds__(256) k_collide_pull(const T* __restrict__ h, T
     }
 }
 
+// ----------------------------------------------------------------------------------------
+// later operators on the two-pass path: colour-gradient collision and moving walls
+// ----------------------------------------------------------------------------------------
+// pass 1 of the colour-gradient step: Theta = (rho^1 - rho^2) / (rho^1 + rho^2); 0 on solid and empty nodes (reading C1)
+template <typename T>
+__global__ void __launch_bounds__(256) k_phase_field(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
+                                                     int nx, int ny, int nz, T* __restrict__ theta) {
+    const long long N = (long long)nx * ny * nz;
+    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    const unsigned lk = links ? links[n] : 0u;
+    T th = T(0);
+    if (!(lk & SOLID_BIT)) {
+        const Nbr b = neighbours(n, nx, ny, nz);
+        T r[2];
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+            T fk[Q], ax, ay, az;
+            pull19<T>(h, NP, k, n, b, lk, fk);
+            moments19<T>(fk, r[k], ax, ay, az);
+        }
+        const T rt = r[0] + r[1];
+        if (rt != T(0)) th = (r[0] - r[1]) / rt;
+    }
+    theta[n] = th;
+}
+
+struct SphereView {
+    const double* c; const double* v; const double* w;     // [p][3] centres, velocities, angular velocities
+    double* F; double* T;                                  // [p][3] accumulators of this step (fp64 for both dtypes)
+    const int* pid;                                        // sphere of every solid node, -1 = a solid at rest that is no sphere
+};
+
+// B_i of PAPER.md:393-398
+template <typename T> __host__ __device__ constexpr T b_rest() { return T(-2.0 / 9.0); }
+template <typename T> __host__ __device__ constexpr T b_pair(int p) { return p < 3 ? T(1.0 / 54.0) : T(1.0 / 27.0); }
+
+// pass 2 for both collision operators, with optional moving walls.
+//   MODEL 0: Shan-Chen as k_collide_pull (aux = rho[2][NP]).
+//   MODEL 1: colour gradient (readings C1-C6 of DESIGN.md section 3), aux = Theta[NP]:
+//            u by Eq. 7, omega from the mean viscosity, BGK (Eq. 9-10), perturbation (Eq. 17, A by Eq. 19),
+//            recolouring (Eq. 20-21).
+//   MOVING:  a link i into a sphere with velocity u_b = v_p + r_b x omega_p (Eq. 22) returns f*_i - 2 rho^k w_i u_b.c_i / c_s^2
+//            (Eq. 24) and hands c_i (f*_i + that) to the sphere (Eq. 25-27; readings M1-M4).  The value is stored where the
+//            plain bounce-back finds it: in the node's own slot i of the post-collision state.
+template <typename T, int MODEL, bool MOVING>
+__global__ void __launch_bounds__(256) k_collide_next(const T* __restrict__ h, T* __restrict__ g, const T* __restrict__ aux,
+                                                      const unsigned* __restrict__ links, long long NP, int nx, int ny, int nz,
+                                                      T om_r, T om_b, T G, T sigma, T beta, T nu_r, T nu_b, SphereView sp) {
+    const long long N = (long long)nx * ny * nz;
+    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+    if (n >= N) return;
+    const unsigned lk = links ? links[n] : 0u;
+    if (lk & SOLID_BIT) return;
+    const Nbr b = neighbours(n, nx, ny, nz);
+    T fr[Q], fb[Q];
+    pull19<T>(h, NP, 0, n, b, lk, fr);
+    pull19<T>(h, NP, 1, n, b, lk, fb);
+    T rr, rb, jrx, jry, jrz, jbx, jby, jbz;
+    moments19<T>(fr, rr, jrx, jry, jrz);
+    moments19<T>(fb, rb, jbx, jby, jbz);
+    if (MODEL == 0) {
+        const T den = om_r * rr + om_b * rb;
+        const T inv = den != T(0) ? T(1) / den : T(0);
+        const T ux = (om_r * jrx + om_b * jbx) * inv, uy = (om_r * jry + om_b * jby) * inv, uz = (om_r * jrz + om_b * jbz) * inv;
+        T gr[3] = {T(0), T(0), T(0)}, gb[3] = {T(0), T(0), T(0)};
+#pragma unroll
+        for (int p = 0; p < 9; ++p) {
+            const long long np = b.at(pair_cx(p), pair_cy(p), pair_cz(p)), nm = b.at(-pair_cx(p), -pair_cy(p), -pair_cz(p));
+            const T db = w_pair<T>(p) * (aux[NP + np] - aux[NP + nm]);
+            const T dr = w_pair<T>(p) * (aux[np] - aux[nm]);
+            if (pair_cx(p)) { gr[0] += T(pair_cx(p)) * db; gb[0] += T(pair_cx(p)) * dr; }
+            if (pair_cy(p)) { gr[1] += T(pair_cy(p)) * db; gb[1] += T(pair_cy(p)) * dr; }
+            if (pair_cz(p)) { gr[2] += T(pair_cz(p)) * db; gb[2] += T(pair_cz(p)) * dr; }
+        }
+        collide19<T>(fr, rr, T(1) - om_r, ux, uy, uz, ux - G * gr[0], uy - G * gr[1], uz - G * gr[2]);
+        collide19<T>(fb, rb, T(1) - om_b, ux, uy, uz, ux - G * gb[0], uy - G * gb[1], uz - G * gb[2]);
+    } else {
+        const T rt = rr + rb;
+        if (rt == T(0)) {                                                   // reading C6
+#pragma unroll
+            for (int i = 0; i < Q; ++i) { fr[i] = T(0); fb[i] = T(0); }
+        } else {
+            const T irt = T(1) / rt;
+            const T ux = (jrx + jbx) * irt, uy = (jry + jby) * irt, uz = (jrz + jbz) * irt;      // Eq. 7
+            const T xr = rr * irt, xb = rb * irt;
+            const T om = T(2) / (T(6) / (xr / nu_r + xb / nu_b) + T(1));                       // PAPER.md:336, reading C2
+            const T A = T(2.25) * sigma * om;                                                  // Eq. 19
+            T gx = T(0), gy = T(0), gz = T(0);                                                 // grad Theta, reading C1
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                const T d = w_pair<T>(p) * (aux[b.at(pair_cx(p), pair_cy(p), pair_cz(p))] - aux[b.at(-pair_cx(p), -pair_cy(p), -pair_cz(p))]);
+                if (pair_cx(p)) gx += T(pair_cx(p)) * d;
+                if (pair_cy(p)) gy += T(pair_cy(p)) * d;
+                if (pair_cz(p)) gz += T(pair_cz(p)) * d;
+            }
+            gx *= T(3); gy *= T(3); gz *= T(3);
+            const T g2 = gx * gx + gy * gy + gz * gz;
+            const T gn = sqrt(g2);
+            const T ig2 = g2 != T(0) ? T(1) / g2 : T(0), ign = g2 != T(0) ? T(1) / gn : T(0);
+            const T amp = T(0.5) * A * gn;                                                     // (A / 2) |grad|, 0 without a gradient
+            const T rc = beta * xr * xb * rt;                                                  // beta rho^1 rho^2 / rho^2 times rho of f^{eq,0}
+            const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+            {   // rest direction: cos(phi) = 0
+                const T fstar = (T(1) - om) * (fr[0] + fb[0]) + om * w_rest<T>() * rt * a0 + T(2) * amp * (-b_rest<T>());
+                fr[0] = xr * fstar; fb[0] = xb * fstar;
+            }
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                const T cu = cdot<T>(p, ux, uy, uz), cg = cdot<T>(p, gx, gy, gz);
+                const T wr = w_pair<T>(p) * rt;
+                const T s0 = a0 + T(4.5) * cu * cu;
+                const T pert = T(2) * amp * (w_pair<T>(p) * cg * cg * ig2 - b_pair<T>(p));      // both components' Eq. 17, same for i and opp(i)
+                const T recol = rc * w_pair<T>(p) * cg * ign * (p < 3 ? T(1) : T(0.70710678118654752440));   // cos(phi_i) = c_i.grad / (|c_i| |grad|)
+                const T f1 = (T(1) - om) * (fr[2 * p + 1] + fb[2 * p + 1]) + om * wr * (s0 + T(3) * cu) + pert;
+                const T f2 = (T(1) - om) * (fr[2 * p + 2] + fb[2 * p + 2]) + om * wr * (s0 - T(3) * cu) + pert;
+                fr[2 * p + 1] = xr * f1 + recol; fb[2 * p + 1] = xb * f1 - recol;               // Eq. 20-21
+                fr[2 * p + 2] = xr * f2 - recol; fb[2 * p + 2] = xb * f2 + recol;
+            }
+        }
+    }
+    if (MOVING && (lk & 0x7FFFEu)) {
+        const int x = int(n % nx), y = int((n / nx) % ny), z = int(n / ((long long)nx * ny));
+#pragma unroll
+        for (int i = 1; i < Q; ++i) {
+            if (!(lk >> i & 1u)) continue;
+            const int p = sp.pid[b.at(dir_cx(i), dir_cy(i), dir_cz(i))];
+            if (p < 0) continue;
+            double rbv[3] = {x + 0.5 * dir_cx(i) - sp.c[3 * p], y + 0.5 * dir_cy(i) - sp.c[3 * p + 1], z + 0.5 * dir_cz(i) - sp.c[3 * p + 2]};
+            rbv[0] -= nx * floor(rbv[0] / nx + 0.5); rbv[1] -= ny * floor(rbv[1] / ny + 0.5); rbv[2] -= nz * floor(rbv[2] / nz + 0.5);
+            const double ub[3] = {sp.v[3 * p] + (rbv[1] * sp.w[3 * p + 2] - rbv[2] * sp.w[3 * p + 1]),      // Eq. 22 as printed
+                                  sp.v[3 * p + 1] + (rbv[2] * sp.w[3 * p] - rbv[0] * sp.w[3 * p + 2]),
+                                  sp.v[3 * p + 2] + (rbv[0] * sp.w[3 * p + 1] - rbv[1] * sp.w[3 * p])};
+            const T wi = i < 7 ? T(1.0 / 18.0) : T(1.0 / 36.0);
+            const T ubi = T(3) * T(ub[0] * dir_cx(i) + ub[1] * dir_cy(i) + ub[2] * dir_cz(i));
+            const T br = fr[i] - T(2) * rr * wi * ubi, bb = fb[i] - T(2) * rb * wi * ubi;            // Eq. 24
+            const double m = (double(fr[i]) + double(br)) + (double(fb[i]) + double(bb));            // momentum handed over along c_i
+            fr[i] = br; fb[i] = bb;
+            const double Fv[3] = {m * dir_cx(i), m * dir_cy(i), m * dir_cz(i)};
+            if (dir_cx(i)) atomicAdd(sp.F + 3 * p, Fv[0]);
+            if (dir_cy(i)) atomicAdd(sp.F + 3 * p + 1, Fv[1]);
+            if (dir_cz(i)) atomicAdd(sp.F + 3 * p + 2, Fv[2]);
+            atomicAdd(sp.T + 3 * p, Fv[1] * rbv[2] - Fv[2] * rbv[1]);                                 // Eq. 27 as printed: F x r_b
+            atomicAdd(sp.T + 3 * p + 1, Fv[2] * rbv[0] - Fv[0] * rbv[2]);
+            atomicAdd(sp.T + 3 * p + 2, Fv[0] * rbv[1] - Fv[1] * rbv[0]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < Q; ++i) {
+        plane(g, NP, 0, i)[n] = fr[i];
+        plane(g, NP, 1, i)[n] = fb[i];
+    }
+}
+
 inline unsigned blocks_for(long long cnt, int bs) { return unsigned((cnt + bs - 1) / bs); }
 
 bool onepass_ok(const lb_ctx* c) { return c->nx % OP_TX == 0 && c->ny % OP_TY == 0; }
@@ -450,6 +612,44 @@ int step_twopass(lb_ctx* c) {
     else
         k_collide_pull<T, false><<<nb, 256, 0, c->stream>>>(h, g, rho, nullptr, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
     c->launches += 1;
+    CU(cudaGetLastError());
+    c->cur ^= 1;
+    c->rho_valid = false;
+    c->hx_valid = false;
+    c->diag_fresh = false;
+    return LB_OK;
+}
+
+SphereView sphere_view(const lb_ctx* c) {
+    SphereView v;
+    v.c = c->sph; v.v = c->sph + 3 * c->nsph; v.w = c->sph + 6 * c->nsph; v.F = c->sph + 9 * c->nsph; v.T = c->sph + 12 * c->nsph;
+    v.pid = c->pid;
+    return v;
+}
+
+// one step of the later operators: colour gradient and / or moving walls, any box shape
+template <typename T>
+int step_next(lb_ctx* c) {
+    const T* h = static_cast<const T*>(c->f[c->cur]);
+    T* g = static_cast<T*>(c->f[c->cur ^ 1]);
+    T* aux = static_cast<T*>(c->rho_in[c->rcur]);
+    const unsigned* lk = c->has_solid ? c->links : nullptr;
+    const unsigned nb = blocks_for(c->N, 256);
+    if (c->model == LB_MODEL_COLOUR_GRADIENT) k_phase_field<T><<<nb, 256, 0, c->stream>>>(h, lk, c->NP, c->nx, c->ny, c->nz, aux);
+    else k_density<T><<<nb, 256, 0, c->stream>>>(h, lk, c->NP, c->nx, c->ny, c->nz, aux);
+    const bool moving = c->nsph > 0;
+    SphereView sp = {};
+    if (moving) {
+        sp = sphere_view(c);
+        CU(cudaMemsetAsync(sp.F, 0, size_t(6) * c->nsph * sizeof(double), c->stream));
+    }
+    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G), sg = T(c->sigma), be = T(c->beta);
+    const T nu_r = T((c->tau[0] - 0.5) / 3.0), nu_b = T((c->tau[1] - 0.5) / 3.0);
+#define LB_NEXT(MODEL, MOVING) k_collide_next<T, MODEL, MOVING><<<nb, 256, 0, c->stream>>>(h, g, aux, lk, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G, sg, be, nu_r, nu_b, sp)
+    if (c->model == LB_MODEL_COLOUR_GRADIENT) { if (moving) LB_NEXT(1, true); else LB_NEXT(1, false); }
+    else { if (moving) LB_NEXT(0, true); else LB_NEXT(0, false); }
+#undef LB_NEXT
+    c->launches += 2;
     CU(cudaGetLastError());
     c->cur ^= 1;
     c->rho_valid = false;
@@ -755,7 +955,10 @@ int resolve_kernel(lb_ctx* c, int kind) {
     return kind;
 }
 
-int effective_kernel(const lb_ctx* c) { return c->kernel == LB_KERNEL_HALO && c->has_solid ? LB_KERNEL_TMA : c->kernel; }
+int effective_kernel(const lb_ctx* c) {
+    if (c->model != LB_MODEL_SHAN_CHEN || c->nsph > 0) return LB_KERNEL_TWOPASS;     // the later operators: general two-pass path
+    return c->kernel == LB_KERNEL_HALO && c->has_solid ? LB_KERNEL_TMA : c->kernel;
+}
 
 long long round64(long long v) { return (v + 63) / 64 * 64; }
 
@@ -869,6 +1072,7 @@ void lb_destroy(lb_ctx* c) {
         cudaFree(c->rho_er[r]); cudaFree(c->rho_ec[r]); cudaFree(c->hx[r]);
     }
     cudaFree(c->stage); cudaFree(c->diag_part); cudaFree(c->diag_out); cudaFree(c->diag_cta);
+    cudaFree(c->sph); cudaFree(c->pid);
     if (c->own_stream) cudaStreamDestroy(c->stream);
     delete c;
 }
@@ -956,6 +1160,7 @@ int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
     if (own_tmp) cudaFree(d_mask);
     if (e != cudaSuccess) return fail_cuda(e, "lb_set_solid_mask");
     c->has_solid = any_solid;   // a mask without solid nodes keeps the plain (no link word) kernels
+    if (!c->in_set_spheres) c->nsph = 0;   // a plain mask: every solid at rest
     c->rho_valid = false;
     if (!any_solid) {
         if (c->have_fields) return c->dtype == LB_F64 ? unstream_scratch<double>(c) : unstream_scratch<float>(c);
@@ -966,6 +1171,84 @@ int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
     if (rc != LB_OK) return rc;
     if (c->have_fields) return f64 ? unstream_scratch<double>(c) : unstream_scratch<float>(c);
     return f64 ? zero_solids<double>(c, c->cur) : zero_solids<float>(c, c->cur);
+}
+
+int lb_set_colour_gradient(lb_ctx* c, double sigma, double beta) {
+    if (!c) return fail(LB_EINVAL, "NULL context");
+    if (!std::isfinite(sigma) || !std::isfinite(beta) || beta < 0.0 || beta > 1.0) return fail(LB_EINVAL, "sigma must be finite, beta in [0, 1]");
+    c->model = LB_MODEL_COLOUR_GRADIENT; c->sigma = sigma; c->beta = beta;
+    c->rho_valid = false;
+    return LB_OK;
+}
+
+int lb_set_shan_chen(lb_ctx* c) {
+    if (!c) return fail(LB_EINVAL, "NULL context");
+    c->model = LB_MODEL_SHAN_CHEN;
+    c->rho_valid = false;
+    return LB_OK;
+}
+
+int lb_set_spheres(lb_ctx* c, int np, const double* centres, double radius, const double* vel, const double* omega) {
+    if (!c || np < 0 || (np > 0 && (!centres || !(radius > 0.0)))) return fail(LB_EINVAL, "lb_set_spheres: bad arguments");
+    DeviceGuard guard(c->device);
+    // solid mask (reading S9) and the sphere of every solid node: integer work on the host, one pass over the spheres' bounding boxes
+    std::string mask;
+    int* pid = nullptr;
+    try { mask.assign(size_t(c->N), char(0)); pid = new int[size_t(c->N)]; } catch (...) { return fail(LB_ENOMEM, "host allocation failed"); }
+    for (long long n = 0; n < c->N; ++n) pid[n] = -1;
+    const int reach = int(std::floor(radius)) + 1;
+    const int dim[3] = {c->nx, c->ny, c->nz};
+    for (int p = 0; p < np; ++p) {
+        const double* ce = centres + 3 * p;
+        int lo[3], hi[3];
+        for (int a = 0; a < 3; ++a) { lo[a] = int(std::floor(ce[a])) - reach; hi[a] = int(std::floor(ce[a])) + reach + 1; }
+        for (int a = 0; a < 3; ++a) if (hi[a] - lo[a] + 1 > dim[a]) { lo[a] = 0; hi[a] = dim[a] - 1; }
+        for (int z = lo[2]; z <= hi[2]; ++z)
+            for (int y = lo[1]; y <= hi[1]; ++y)
+                for (int x = lo[0]; x <= hi[0]; ++x) {
+                    const int q[3] = {((x % dim[0]) + dim[0]) % dim[0], ((y % dim[1]) + dim[1]) % dim[1], ((z % dim[2]) + dim[2]) % dim[2]};
+                    double d2 = 0.0;
+                    for (int a = 0; a < 3; ++a) {
+                        double d = std::fabs(q[a] - ce[a]);
+                        d = std::fmin(d, dim[a] - d);
+                        d2 += d * d;
+                    }
+                    const long long n = q[0] + (long long)dim[0] * (q[1] + (long long)dim[1] * q[2]);
+                    if (d2 <= radius * radius && pid[n] < 0) { mask[size_t(n)] = 1; pid[n] = p; }
+                }
+    }
+    cudaFree(c->sph); cudaFree(c->pid);
+    c->sph = nullptr; c->pid = nullptr;
+    int rc = LB_OK;
+    if (np > 0) {
+        cudaError_t e = cudaMalloc(&c->sph, size_t(15) * np * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc(&c->pid, size_t(c->N) * sizeof(int));
+        if (e == cudaSuccess) e = cudaMemsetAsync(c->sph, 0, size_t(15) * np * sizeof(double), c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(c->sph, centres, size_t(3) * np * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess && vel) e = cudaMemcpyAsync(c->sph + 3 * np, vel, size_t(3) * np * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess && omega) e = cudaMemcpyAsync(c->sph + 6 * np, omega, size_t(3) * np * sizeof(double), cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(c->pid, pid, size_t(c->N) * sizeof(int), cudaMemcpyHostToDevice, c->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+        if (e != cudaSuccess) rc = fail_cuda(e, "lb_set_spheres");
+    }
+    delete[] pid;
+    if (rc != LB_OK) return rc;
+    c->in_set_spheres = true;
+    rc = lb_set_solid_mask(c, reinterpret_cast<const unsigned char*>(mask.data()));
+    c->in_set_spheres = false;
+    if (rc != LB_OK) return rc;
+    c->nsph = np; c->radius = radius;
+    return LB_OK;
+}
+
+int lb_get_sphere_forces(lb_ctx* c, double* F, double* T) {
+    if (!c || !F || !T) return fail(LB_EINVAL, "NULL argument");
+    if (c->nsph == 0) return LB_OK;
+    DeviceGuard guard(c->device);
+    CU(cudaMemcpyAsync(F, c->sph + 9 * c->nsph, size_t(3) * c->nsph * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaMemcpyAsync(T, c->sph + 12 * c->nsph, size_t(3) * c->nsph * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return LB_OK;
 }
 
 int lb_set_fields(lb_ctx* c, const double* rho_r, const double* rho_b, const double* ux, const double* uy, const double* uz) {
@@ -1037,7 +1320,8 @@ int lb_step(lb_ctx* c, int nsteps) {
     for (int s = 0; s < nsteps; ++s) {
         int rc;
         const int kern = effective_kernel(c);
-        if (kern == LB_KERNEL_HALO) rc = c->dtype == LB_F64 ? step_halo<double>(c) : step_halo<float>(c);
+        if (c->model != LB_MODEL_SHAN_CHEN || c->nsph > 0) rc = c->dtype == LB_F64 ? step_next<double>(c) : step_next<float>(c);
+        else if (kern == LB_KERNEL_HALO) rc = c->dtype == LB_F64 ? step_halo<double>(c) : step_halo<float>(c);
         else if (kern == LB_KERNEL_TMA) rc = c->dtype == LB_F64 ? step_tma<double>(c) : step_tma<float>(c);
         else if (kern == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);
         else rc = c->dtype == LB_F64 ? step_twopass<double>(c) : step_twopass<float>(c);

@@ -456,6 +456,113 @@ def test_single_fluid_random_populations_and_errors(oracle_mod):
 
 
 # ---------------------------------------------------------------------------------------------
+# later operators: colour-gradient collision, moving walls with per-sphere force / torque
+# ---------------------------------------------------------------------------------------------
+def _two_phase(nx, ny, nz, seed):
+    rng = np.random.default_rng(seed)
+    phi = rng.uniform(-0.9, 0.9, nx * ny * nz)
+    rho = 1.0 + 0.05 * rng.uniform(-1, 1, nx * ny * nz)
+    return rho * (1 + phi) / 2, rho * (1 - phi) / 2, rng.uniform(-0.02, 0.02, (3, nx * ny * nz))
+
+
+@pytest.mark.parametrize("dtype,tol", [(B.LB_F64, 1e-13), (B.LB_F32, 2e-5)])
+@pytest.mark.parametrize("shape,tau,sigma,beta,solid", [((32, 32, 32), (1.0, 1.0), 0.02, 0.7, False), ((40, 24, 12), (0.8, 1.4), 0.01, 0.99, True),
+                                                        ((7, 5, 3), (0.7, 0.9), 0.05, 0.3, False), ((64, 16, 8), (0.6, 1.9), 0.0, 0.5, True)])
+def test_colour_gradient_against_oracle(oracle_mod, dtype, tol, shape, tau, sigma, beta, solid):
+    nx, ny, nz = shape
+    rr, rb, u = _two_phase(nx, ny, nz, 31)
+    mask = None
+    if solid:
+        mask = np.zeros((nz, ny, nx), np.uint8)
+        mask[1:3, 2:6, 5:11] = 1
+        mask[nz - 1, 0, 0] = 1
+    o = oracle_mod.Oracle(nx, ny, nz, tau[0], tau[1], 0.0)
+    o.set_colour_gradient(sigma, beta)
+    if solid:
+        o.set_solid_mask(mask)
+    o.set_fields(rr, rb, *u)
+    with B.Box(nx, ny, nz, tau[0], tau[1], 0.0, dtype=dtype) as box:
+        box.set_colour_gradient(sigma, beta)
+        if solid:
+            box.set_solid_mask(mask)
+        box.set_fields(rr, rb, *u)
+        for steps in (1, 4, 25):
+            o.step(steps), box.step(steps)
+            e = nerr(box.get_populations(), o.get_populations())
+            assert e < tol, (steps, e)
+        (gm, gp), (om, op) = box.get_diagnostics(), o.get_diagnostics()
+        assert np.abs(gm / om - 1).max() < (1e-13 if dtype == B.LB_F64 else 1e-5)
+        # and back to Shan-Chen on the same context
+        box.set_shan_chen()
+        o2 = oracle_mod.Oracle(nx, ny, nz, tau[0], tau[1], 0.0)
+        if solid:
+            o2.set_solid_mask(mask)
+        o2.set_populations(o.get_populations())
+        box.set_populations(o.get_populations())
+        o2.step(2), box.step(2)
+        assert nerr(box.get_populations(), o2.get_populations()) < tol
+
+
+def test_colour_gradient_droplet_256_sampled(oracle_mod):
+    """Colour gradient at the paper's box size (256^3, Table 2) from a seeded random colour field: all 38 populations
+    at sampled nodes after 6 steps against the oracle on a cut-out (a node depends on the state within 2 nodes per step)."""
+    n, s, hw = 256, 6, 13
+    cfg = w.CONFIGS[1]
+    rr, rb = cfg.fields()
+    rng_nodes = [(0, 0, 0), (255, 255, 255), (31, 7, 128), (100, 200, 17), (32, 8, 255), (128, 0, 64)]
+    R, Bl = rr.reshape(n, n, n), rb.reshape(n, n, n)
+    with B.Box(n, n, n, 1.0, 1.0, 0.0, dtype=B.LB_F64) as box:
+        box.set_colour_gradient(0.02, 0.7)
+        box.set_fields(rr, rb)
+        box.step(s)
+        f = box.get_populations()
+        for (x, y, z) in rng_nodes:
+            ix, iy, iz = (np.arange(c - hw, c + hw + 1) % n for c in (x, y, z))
+            sub = np.ix_(iz, iy, ix)
+            L = 2 * hw + 1
+            o = oracle_mod.Oracle(L, L, L, 1.0, 1.0, 0.0)
+            o.set_colour_gradient(0.02, 0.7)
+            o.set_fields(np.ascontiguousarray(R[sub]).reshape(-1), np.ascontiguousarray(Bl[sub]).reshape(-1))
+            o.step(s)
+            want = o.get_populations()[:, :, hw, hw, hw]
+            assert np.abs(f[:, :, z, y, x] - want).max() / np.abs(want).max() < 1e-13, (x, y, z)
+
+
+@pytest.mark.parametrize("model", ["sc", "cg"])
+@pytest.mark.parametrize("dtype,tol,ftol", [(B.LB_F64, 1e-13, 1e-11), (B.LB_F32, 2e-5, 2e-4)])
+def test_moving_spheres_against_oracle(oracle_mod, model, dtype, tol, ftol):
+    """Moving-wall bounce-back (Eq. 22-24) and the force / torque on every sphere (Eq. 25-27) against the oracle: translating and
+    rotating spheres, one across the periodic seam; populations every step, forces relative to the largest force."""
+    n = 32
+    centres = np.array([[7.3, 8.1, 6.6], [17.2, 15.9, 16.4], [31.6, 0.4, 15.5]])
+    vel = np.array([[0.02, 0.0, -0.01], [0.0, 0.015, 0.0], [0.0, 0.0, 0.0]])
+    omg = np.array([[0.0, 0.0, 0.004], [0.003, -0.002, 0.0], [0.001, 0.0, 0.002]])
+    # Shan-Chen: the seeded mixture; colour gradient: a field with O(1) colour contrasts (in a nearly mixed fluid cos(phi_i) and
+    # (c_i.grad)^2 / |grad|^2 are ratios of sums ~ 1e-3, whose rounding error is eps / 1e-3: measured 1.6e-13 normalised in fp64)
+    rr, rb = w.mixture_fields(n, n, n, 22) if model == "sc" else _two_phase(n, n, n, 23)[:2]
+    o = oracle_mod.Oracle(n, n, n, 0.9, 1.1, 0.6)
+    o.set_spheres(centres, 4.5, vel, omg)
+    o.set_fields(rr, rb)
+    with B.Box(n, n, n, 0.9, 1.1, 0.6, dtype=dtype) as box:
+        box.set_fields(rr, rb)                                   # other order on purpose
+        box.set_spheres(centres, 4.5, vel, omg)
+        if model == "cg":
+            o.set_colour_gradient(0.01, 0.5), box.set_colour_gradient(0.01, 0.5)
+        assert np.array_equal(box.get_link_mask(), o.get_link_mask())
+        for _ in range(6):
+            o.step(1), box.step(1)
+            assert nerr(box.get_populations(), o.get_populations()) < tol
+            (gF, gT), (oF, oT) = box.get_sphere_forces(), o.get_sphere_forces()
+            assert np.abs(gF - oF).max() < ftol * np.abs(oF).max()
+            assert np.abs(gT - oT).max() < ftol * np.abs(oT).max()
+        # walls at rest again: a plain mask removes the sphere velocities
+        mask = o.get_solid_mask()
+        o.set_solid_mask(mask), box.set_solid_mask(mask)
+        o.step(2), box.step(2)
+        assert nerr(box.get_populations(), o.get_populations()) < tol
+
+
+# ---------------------------------------------------------------------------------------------
 # API behaviour on the device
 # ---------------------------------------------------------------------------------------------
 def test_state_and_argument_errors():
