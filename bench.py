@@ -230,6 +230,9 @@ def run_ours(args):
         if name in SINGLE:
             run_single(args, name, B, torch, dev, rank, local_rank, world)
             continue
+        if args.decomposition == "slab":
+            run_slab(args, with_overrides(WORKLOADS[name], args), B, torch, dev, rank, local_rank, world)
+            continue
         # `all`: the CPU oracle is timed once (on the headline workload), not five times
         cpu = not args.no_cpu_baseline and (args.workload != "all" or name == "config2")
         run_one(args, with_overrides(WORKLOADS[name], args), B, torch, dev, rank, local_rank, world, cpu)
@@ -294,6 +297,64 @@ def run_single(args, name, B, torch, dev, rank, local_rank, world):
         "gpu_launches": launches, "clocks": clocks,
     }
     print(json.dumps(line), flush=True)
+
+
+def run_slab(args, cfg, B, torch, dev, rank, local_rank, world):
+    """--decomposition slab: ONE global box split into z slabs, one per rank, two ghost planes exchanged with the ring
+    neighbours before every step over torch.distributed (NCCL / NVLink): strong scaling.  General two-pass kernels."""
+    from paper_2112_08264_b200 import slab as S
+    import torch.distributed as dist
+    if world == 1 and not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1"); os.environ.setdefault("MASTER_PORT", "29531")
+        dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
+    dtype = B.LB_F64 if cfg.dtype == "f64" else B.LB_F32
+    stream = torch.cuda.current_stream(dev)
+    sl = S.SlabBox(cfg.nx, cfg.ny, cfg.nz, rank, world, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype, cuda_stream=stream.cuda_stream, device=dev)
+    rr, rb = cfg.fields()
+    sl.set_fields(rr, rb)
+    del rr, rb
+    steps, warmup = args.steps, max(args.warmup, 3)
+
+    def advance(k):
+        for _ in range(k):
+            S.ring_exchange_dist(sl, dist)
+            sl.step(1)
+    advance(warmup)
+    torch.cuda.synchronize(dev)
+    dist.barrier()
+    sampler = ClockSampler(local_rank)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = sl.box.launch_count()
+    e0.record(stream)
+    advance(steps)
+    e1.record(stream)
+    e1.synchronize()
+    torch.cuda.synchronize(dev)
+    dist.barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    launches = sl.box.launch_count() - l0
+    ms_max, _ = aggregate_over_ranks(ms, 0.0, world, dev)
+    N = cfg.n_nodes
+    glups = N * steps / (ms_max * 1e-3) / 1e9
+    sl.close()
+    if rank != 0:
+        return
+    es = 8 if cfg.dtype == "f64" else 4
+    halo = 2 * 2 * 38 * S.GHOST * cfg.nx * cfg.ny * es
+    peak, peak_src = measured_peak()
+    alg = ALG_BYTES[cfg.dtype]
+    achieved = alg * N / world / (ms / steps * 1e-3) / 1e9
+    print(json.dumps({
+        "metric": METRIC, "value": glups, "unit": "GLUPS", "n_gpus": world, "steps": steps, "warmup": warmup, "ms_per_step": ms_max / steps,
+        "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": cfg.dtype, "data": "synthetic",
+        "config": {"workload": cfg.name, "box": [cfg.nx, cfg.ny, cfg.nz], "tau": [cfg.tau_r, cfg.tau_b], "G": cfg.G, "kernel": "twopass",
+                   "parallelism": f"z slabs x{world}, {S.GHOST} ghost planes per side exchanged every step (torch.distributed P2P)",
+                   "halo_bytes_per_rank_per_step": halo, "launches_per_step": launches / steps},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes_per_node": alg, "kernel_ms": ms / steps, "kernel": "whole step of one rank"},
+        "e2e": {"value": None, "unit": "GLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "note": "not measured in slab mode"},
+        "gpu_launches": launches, "clocks": clocks}), flush=True)
 
 
 def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
@@ -440,6 +501,8 @@ def main():
     ap.add_argument("--beta", type=float, default=0.7)
     ap.add_argument("--moving-walls", action="store_true", help="config4: spheres with seeded velocities, force / torque per sphere each step")
     ap.add_argument("--f32", action="store_true", help="run the workload in fp32 (e.g. config1 --f32 --model cg: the paper's Table 2 setting)")
+    ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
+                    help="--gpus N: N independent replicas (north_star: the path does not shard) or ONE box in N z slabs with halo exchange (N3)")
     ap.add_argument("--diag", action="store_true", help="per-step mass / momentum sums fused into the step kernel (LB_OPT_DIAG)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma", "halo"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

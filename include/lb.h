@@ -45,7 +45,7 @@ typedef struct lb_ctx lb_ctx;          /* opaque; owned by the library */
 enum { LB_OK = 0, LB_EINVAL = -1, LB_ENOMEM = -2, LB_ECUDA = -3, LB_ESTATE = -4 };
 enum { LB_F64 = 0, LB_F32 = 1 };
 enum { LB_KERNEL_AUTO = 0, LB_KERNEL_TWOPASS = 1, LB_KERNEL_ONEPASS = 2, LB_KERNEL_TMA = 3, LB_KERNEL_HALO = 4 };
-enum { LB_OPT_ZC = 1, LB_OPT_DIAG = 2, LB_OPT_CLUSTER = 3 };
+enum { LB_OPT_ZC = 1, LB_OPT_DIAG = 2 };
 enum { LB_MODEL_SHAN_CHEN = 0, LB_MODEL_COLOUR_GRADIENT = 1 };   /* options of lb_set_option */
 
 /* Create a context for an nx*ny*nz periodic box holding two fluids with BGK
@@ -124,7 +124,7 @@ int lb_get_diagnostics(lb_ctx* ctx, double mass[2], double momentum[3]);
  * TMA-staged single pass that reads aligned tiles only (the x neighbour's column comes from
  * x-halo copies) and sums the density of the tile's own nodes from the staged populations
  * instead of carrying it (less DRAM traffic, measured slower; no bounce-back: a box with solid
- * nodes runs LB_KERNEL_TMA instead; the only kernel with LB_OPT_DIAG); LB_KERNEL_AUTO (default)
+ * nodes runs LB_KERNEL_TMA instead; ); LB_KERNEL_AUTO (default)
  * = TMA when the box shape allows it (ONEPASS if the driver cannot encode the tensor maps), else
  * TWOPASS: boxes whose sides are not multiples of the 32 x 8 tile run about 1.5 x slower.
  * LB_EINVAL if the box shape does not allow `kind`. */
@@ -135,14 +135,13 @@ int lb_get_kernel(const lb_ctx* ctx);
 
 /* Tuning and modes.  LB_OPT_ZC: planes per CTA of the one-pass kernels (each CTA marches over
  * value z planes and re-collides one more at either end); 0 = the library's heuristic (default).
- * LB_OPT_DIAG (0 / 1, default 0): per-step diagnostics fused into the step: with LB_KERNEL_HALO
- * every lb_step leaves the per-component mass and the total momentum of the NEW state behind
- * (per thread in shared memory, warp shuffles, one partial per CTA, added in a fixed order), and
- * lb_get_diagnostics then makes no pass over the populations; the momentum is the sum of the
- * post-collision moments (1 - omega_k) j^k + omega_k rho^k u' + rho^k du^k, which streaming in a
- * periodic box only permutes.  With any other kernel the option changes nothing.
- * LB_OPT_CLUSTER (1..8, default 1): launch LB_KERNEL_TMA in thread-block clusters of that many
- * x-adjacent tiles (measured: no gain).
+ * LB_OPT_DIAG (0 / 1, default 0): per-step diagnostics fused into the step: with LB_KERNEL_TMA and
+ * LB_KERNEL_HALO on a box without solid nodes, every lb_step leaves the per-component mass and the
+ * total momentum of the NEW state behind (warp-shuffle reductions, one partial per CTA, added in
+ * a fixed order: deterministic), and lb_get_diagnostics then makes no pass over the populations;
+ * the momentum is the sum of the post-collision moments (1 - omega_k) j^k + omega_k rho^k u' +
+ * rho^k du^k, which streaming in a periodic box only permutes.  Otherwise (solid nodes, other
+ * kernels, other operators) lb_get_diagnostics makes its own pass as before.
  * LB_EINVAL for an unknown option or a value out of range.  lb_get_option returns the value in
  * effect (for LB_OPT_ZC: the planes per CTA the current kernel will use), -1 on error. */
 int lb_set_option(lb_ctx* ctx, int option, long long value);
@@ -188,6 +187,19 @@ int lb_set_shan_chen(lb_ctx* ctx);
  * lb_set_solid_mask afterwards also makes every solid a wall at rest again.  Synchronises. */
 int lb_set_spheres(lb_ctx* ctx, int np, const double* centres, double radius, const double* vel, const double* omega);
 int lb_get_sphere_forces(lb_ctx* ctx, double* F, double* T);
+
+/* ---- slab decomposition ("equal sub-domains ... border exchange"; Tables 4-5) ----------------
+ * The box of one context can be a z slab of a larger periodic box with two ghost planes on either side: run lb_step on
+ * the slab as it is (its own periodic wrap only ever feeds the outermost ghost planes, whose results are thrown away)
+ * and, before every step, overwrite the ghost planes with the neighbour slabs' outermost interior planes.  These two
+ * calls move whole z planes [z0, z0 + nplanes) of the device state (the 38 population planes in the library's private
+ * order and type: 38 * nplanes * nx * ny values of 8 or 4 bytes) to / from a caller-owned DEVICE buffer, on the
+ * context's stream, asynchronously: the caller ships the buffer to the neighbour rank (NCCL / peer copy over NVLink)
+ * on the same stream or after lb_sync.  An import invalidates the carried density, so the one-pass kernels pay a
+ * density pass after it; the two-pass path is unaffected.  paper_2112_08264_b200/slab.py drives this.
+ * LB_EINVAL if the range leaves the box, LB_ESTATE before any state was set. */
+int lb_export_planes(lb_ctx* ctx, int z0, int nplanes, void* device_dst);
+int lb_import_planes(lb_ctx* ctx, int z0, int nplanes, const void* device_src);
 
 /* ---- single-fluid calibration path (the paper's case 1, Table 1) --------------
  * One BGK fluid on the same D3Q19 lattice, periodic box, no force, no solids, fused collide +

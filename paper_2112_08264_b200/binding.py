@@ -17,7 +17,8 @@ import numpy as np
 LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 LB_F64, LB_F32 = 0, 1
 LB_KERNEL_AUTO, LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA, LB_KERNEL_HALO = 0, 1, 2, 3, 4
-LB_OPT_ZC, LB_OPT_DIAG, LB_OPT_CLUSTER = 1, 2, 3
+LB_OPT_ZC, LB_OPT_DIAG = 1, 2
+LB_MODEL_SHAN_CHEN, LB_MODEL_COLOUR_GRADIENT = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "_lib", "liblb_b200.so")
@@ -29,6 +30,7 @@ SYMBOLS = (
     "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
     "lb_set_option", "lb_get_option", "lb_sync", "lb_last_error", "lb_last_error_code", "lb_version",
     "lb_set_colour_gradient", "lb_set_shan_chen", "lb_set_spheres", "lb_get_sphere_forces",
+    "lb_export_planes", "lb_import_planes",
     "lbs_create", "lbs_destroy", "lbs_set_fields", "lbs_set_populations", "lbs_step", "lbs_get_populations",
     "lbs_get_moments", "lbs_sync", "lbs_launch_count",
 )
@@ -81,6 +83,8 @@ def lib() -> C.CDLL:
     L.lb_set_shan_chen.argtypes = [C.c_void_p]
     L.lb_set_spheres.argtypes = [C.c_void_p, C.c_int, _dp, C.c_double, _dp, _dp]
     L.lb_get_sphere_forces.argtypes = [C.c_void_p, _dp, _dp]
+    L.lb_export_planes.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+    L.lb_import_planes.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
     L.lbs_create.restype = C.c_void_p
     L.lbs_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p]
     L.lbs_destroy.restype = None
@@ -278,6 +282,12 @@ class Box:
         v = None if vel is None else _host_f64(vel, 3 * self.nsph, "vel")
         w = None if omega is None else _host_f64(omega, 3 * self.nsph, "omega")
         _chk(lib().lb_set_spheres(self.h, self.nsph, _d(c.reshape(-1)), radius, _d(v), _d(w)))
+
+    def export_planes(self, z0, nplanes, device_ptr):
+        _chk(lib().lb_export_planes(self.h, z0, nplanes, device_ptr))
+
+    def import_planes(self, z0, nplanes, device_ptr):
+        _chk(lib().lb_import_planes(self.h, z0, nplanes, device_ptr))
 
     def get_sphere_forces(self):
         F, T = np.zeros(3 * self.nsph), np.zeros(3 * self.nsph)

@@ -68,7 +68,6 @@ struct lb_ctx {
     double radius;
     double* sph;       // device: centres[nsph][3], vel[nsph][3], omega[nsph][3], F[nsph][3], T[nsph][3]
     int* pid;          // device: sphere of every solid node (-1 = none)
-    int cluster_x;     // LB_OPT_CLUSTER: thread-block cluster size along x for the TMA kernel (1 = none)
     int diag_mode;     // LB_OPT_DIAG: the halo kernel also leaves the mass / momentum sums of the new state behind
     bool diag_fresh;   // diag_cta holds the per-CTA partials of the state in f[cur]
     double* diag_cta;  // [diag_cta_cap][5]
@@ -786,29 +785,32 @@ bool make_tmaps(lb_ctx* c) {
     return true;
 }
 
-template <typename T, bool HAS_SOLID>
+int ensure_diag_buf(lb_ctx* c, long long ncta) {
+    if (c->diag_cta && c->diag_cta_cap >= ncta) return LB_OK;
+    CU(cudaStreamSynchronize(c->stream));
+    cudaFree(c->diag_cta);
+    c->diag_cta = nullptr;
+    CU(cudaMalloc(&c->diag_cta, size_t(ncta) * 5 * sizeof(double)));
+    c->diag_cta_cap = ncta;
+    return LB_OK;
+}
+
+template <typename T, bool HAS_SOLID, bool DIAG>
 int launch_tma(lb_ctx* c) {
-    auto kern = k_step_tma<T, HAS_SOLID, OP_TY>;
+    auto kern = k_step_tma<T, HAS_SOLID, OP_TY, DIAG>;
     constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
     const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
-    if (c->cluster_x > 1 && grid.x % c->cluster_x == 0) {
-        // thread-block clusters along x: the CTAs of x-adjacent tiles start together, so the 16-byte box margins one of them reads
-        // are the other's own tile data of the same plane
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = grid; cfg.blockDim = dim3(2 * OP_TX * OP_TY + 128); cfg.dynamicSmemBytes = smem; cfg.stream = c->stream;
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = unsigned(c->cluster_x); at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
-        CU(cudaLaunchKernelEx(&cfg, kern, c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
-                              static_cast<T*>(c->f[c->cur ^ 1]), static_cast<const unsigned*>(HAS_SOLID ? c->links : nullptr),
-                              rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz, c->zc_tma, om_r, om_b, G));
-    } else
+    if (DIAG) {
+        const long long ncta = (long long)grid.x * grid.y * grid.z;
+        const int rc = ensure_diag_buf(c, ncta);
+        if (rc != LB_OK) return rc;
+        c->diag_ncta = ncta;
+    }
     kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                            static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                            rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
-                                                           c->zc_tma, om_r, om_b, G);
+                                                           c->zc_tma, om_r, om_b, G, c->diag_cta);
     c->launches += 1;
     CU(cudaGetLastError());
     return LB_OK;
@@ -818,12 +820,13 @@ template <typename T>
 int step_tma(lb_ctx* c) {
     int rc = ensure_rho<T>(c);
     if (rc != LB_OK) return rc;
-    rc = c->has_solid ? launch_tma<T, true>(c) : launch_tma<T, false>(c);
+    const bool diag = c->diag_mode && !c->has_solid;        // with bounce-back the walls take momentum: the separate pass does it
+    rc = c->has_solid ? launch_tma<T, true, false>(c) : (diag ? launch_tma<T, false, true>(c) : launch_tma<T, false, false>(c));
     if (rc != LB_OK) return rc;
     c->cur ^= 1;
     c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
     c->hx_valid = false;
-    c->diag_fresh = false;
+    c->diag_fresh = diag;
     return LB_OK;
 }
 
@@ -867,15 +870,6 @@ int ensure_halo_state(lb_ctx* c) {
     return LB_OK;
 }
 
-int ensure_diag_buf(lb_ctx* c, long long ncta) {
-    if (c->diag_cta && c->diag_cta_cap >= ncta) return LB_OK;
-    CU(cudaStreamSynchronize(c->stream));
-    cudaFree(c->diag_cta);
-    c->diag_cta = nullptr;
-    CU(cudaMalloc(&c->diag_cta, size_t(ncta) * 5 * sizeof(double)));
-    c->diag_cta_cap = ncta;
-    return LB_OK;
-}
 
 template <typename T, bool DIAG>
 int launch_halo(lb_ctx* c) {
@@ -918,6 +912,7 @@ int configure_onepass_kernels() {
     CU(cudaFuncSetAttribute(k_step_pull<T, true, OP_TX, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(onepass_smem_bytes<T, OP_TX, OP_TY>())));
     CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_tma<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
+    CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_halo<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<false>())));
     CU(cudaFuncSetAttribute(k_step_halo<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<true>())));
     return LB_OK;
@@ -1050,7 +1045,6 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
         return nullptr;                                  // LB_ECUDA, message set
     }
     c->have_tmap = onepass_ok(c) && make_tmaps(c);
-    c->cluster_x = 1;
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
     c->zc = onepass_zc(c);
@@ -1098,10 +1092,6 @@ int lb_set_option(lb_ctx* c, int option, long long value) {
         c->zc = onepass_zc(c);
         c->zc_tma = tma_zc(c);
         return LB_OK;
-    case LB_OPT_CLUSTER:
-        if (value < 1 || value > 8) return fail(LB_EINVAL, "LB_OPT_CLUSTER: 1..8");
-        c->cluster_x = int(value);
-        return LB_OK;
     case LB_OPT_DIAG:
         if (value != 0 && value != 1) return fail(LB_EINVAL, "LB_OPT_DIAG: 0 or 1");
         c->diag_mode = int(value);
@@ -1117,7 +1107,6 @@ long long lb_get_option(const lb_ctx* c, int option) {
     switch (option) {
     case LB_OPT_ZC: return (c->kernel == LB_KERNEL_TMA || c->kernel == LB_KERNEL_HALO) ? c->zc_tma : c->zc;
     case LB_OPT_DIAG: return c->diag_mode;
-    case LB_OPT_CLUSTER: return c->cluster_x;
     default: return -1;
     }
 }
@@ -1240,6 +1229,26 @@ int lb_set_spheres(lb_ctx* c, int np, const double* centres, double radius, cons
     c->nsph = np; c->radius = radius;
     return LB_OK;
 }
+
+// ---- slab decomposition: whole z planes of the device state to / from a caller-owned DEVICE buffer ----
+static int plane_copy(lb_ctx* c, int z0, int nplanes, void* dev, bool out) {
+    if (!c || !dev) return fail(LB_EINVAL, "NULL argument");
+    if (z0 < 0 || nplanes < 1 || z0 + nplanes > c->nz) return fail(LB_EINVAL, "plane range outside the box (no wrap)");
+    if (!c->have_fields) return fail(LB_ESTATE, "no state to exchange yet");
+    DeviceGuard guard(c->device);
+    const size_t es = esize(c), pl = size_t(c->nx) * c->ny, width = size_t(nplanes) * pl * es;
+    char* state = static_cast<char*>(c->f[c->cur]) + size_t(z0) * pl * es;
+    if (out) CU(cudaMemcpy2DAsync(dev, width, state, size_t(c->NP) * es, width, NPOP, cudaMemcpyDeviceToDevice, c->stream));
+    else {
+        CU(cudaMemcpy2DAsync(state, size_t(c->NP) * es, dev, width, width, NPOP, cudaMemcpyDeviceToDevice, c->stream));
+        c->rho_valid = false;                    // the carried density / x-halo copies / fused sums no longer describe the state
+        c->hx_valid = false;
+        c->diag_fresh = false;
+    }
+    return LB_OK;
+}
+int lb_export_planes(lb_ctx* c, int z0, int nplanes, void* device_dst) { return plane_copy(c, z0, nplanes, device_dst, true); }
+int lb_import_planes(lb_ctx* c, int z0, int nplanes, const void* device_src) { return plane_copy(c, z0, nplanes, const_cast<void*>(device_src), false); }
 
 int lb_get_sphere_forces(lb_ctx* c, double* F, double* T) {
     if (!c || !F || !T) return fail(LB_EINVAL, "NULL argument");

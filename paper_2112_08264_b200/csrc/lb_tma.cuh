@@ -128,7 +128,8 @@ struct TmaLayout {
     static constexpr size_t BAR_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
     // mbarriers: full[2], done[2], rdy, rowpub[2][2 TY]
     static constexpr int NBARS = 5 + 4 * TY;
-    static constexpr size_t BYTES = BAR_BYTE_OFF + NBARS * sizeof(unsigned long long);
+    static constexpr size_t WACC_BYTE_OFF = BAR_BYTE_OFF + NBARS * sizeof(unsigned long long);   // double [2 TY][4]: per-warp sums (DIAG)
+    static constexpr size_t BYTES = WACC_BYTE_OFF + 2 * TY * 4 * sizeof(double);
     static_assert(BYTES <= 227 * 1024, "shared memory per CTA");
 };
 
@@ -138,12 +139,17 @@ struct TmaLayout {
 // Threads: 2*NT consumers (component k = t / NT, node (tx, ty) = ((t % NT) % 32, (t % NT) / 32): one warp per
 // tile row and component) followed by one producer warp group (TMA warp + 3 ring warps).  The producer
 // group gives its registers to the consumers (setmaxnreg), which is why it is a whole warp group.
-template <typename T, bool HAS_SOLID, int TY>
+// DIAG (boxes without solids): the kernel also leaves the per-component mass and the total momentum of the state AFTER this step
+// behind, one partial per CTA: the post-collision moments sum_i f*_i = rho, sum_i f*_i c_i = (1 - om) j + om rho u' + rho du
+// (Eq. 1, Eq. 10, S5), which streaming in a periodic box only permutes.  Per plane a four-value warp reduction (6 shuffles of
+// doubles) into per-warp shared-memory sums; at the end the 2 TY warp sums in a fixed order.
+template <typename T, bool HAS_SOLID, int TY, bool DIAG = false>
 __global__ void __launch_bounds__(2 * 32 * TY + 128, 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
            const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
-           T om_r, T om_b, T G) {
+           T om_r, T om_b, T G, double* __restrict__ diag_part = nullptr) {
+    static_assert(!(DIAG && HAS_SOLID), "the fused sums assume periodic streaming without bounce-back");
     using L = TmaLayout<T, TY>;
     constexpr int TX = L::TX, NT = L::NT, NC = 2 * NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     static_assert(TY >= 2 && TY <= 8, "one named barrier per tile row (ids 1..TY)");
@@ -450,6 +456,26 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             const T G_ = cst[2];
             ex = ux - G_ * gx; ey = uy - G_ * gy; ez = uz - G_ * gz;
         }
+        if (DIAG) {
+            const double om = 1.0 - double(omc), r_ = store_h ? double(rho) : 0.0;      // the re-collided planes belong to another chunk
+            double v0 = r_, v1 = r_ == 0.0 ? 0.0 : double(omc) * double(jx) + r_ * (om * double(ux) + (double(ex) - double(ux)));
+            double v2 = r_ == 0.0 ? 0.0 : double(omc) * double(jy) + r_ * (om * double(uy) + (double(ey) - double(uy)));
+            double v3 = r_ == 0.0 ? 0.0 : double(omc) * double(jz) + r_ * (om * double(uz) + (double(ez) - double(uz)));
+            // four values, 32 lanes: two halving steps, then three plain ones; lanes 0, 8, 16, 24 end up with the sums of v0, v1, v2, v3
+            const bool hA = (tx & 16) != 0, hB = (tx & 8) != 0;
+            double kA = hA ? v2 : v0, kB = hA ? v3 : v1;
+            kA += __shfl_xor_sync(0xffffffffu, hA ? v0 : v2, 16);
+            kB += __shfl_xor_sync(0xffffffffu, hA ? v1 : v3, 16);
+            double kk_ = hB ? kB : kA;
+            kk_ += __shfl_xor_sync(0xffffffffu, hB ? kA : kB, 8);
+            kk_ += __shfl_xor_sync(0xffffffffu, kk_, 4);
+            kk_ += __shfl_xor_sync(0xffffffffu, kk_, 2);
+            kk_ += __shfl_xor_sync(0xffffffffu, kk_, 1);
+            if ((tx & 7) == 0) {
+                double* wa = reinterpret_cast<double*>(smem_tma + L::WACC_BYTE_OFF) + (t / 32) * 4 + (hA ? 2 : 0) + (hB ? 1 : 0);
+                *wa = (it == 0 ? 0.0 : *wa) + kk_;
+            }
+        }
 
         // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5), and, pair by pair as the post-collision values
         //      appear: their (aligned, coalesced) stores and the x stage of the density gather
@@ -569,6 +595,17 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         zt = zl;
         zl = zl + 1 == nz ? 0 : zl + 1;
         if (HAS_SOLID && it + 1 < niter) lk = __ldg(links + (e_own - unsigned(k * NP)) + (long long)zl * pl);
+    }
+    if (DIAG) {
+        asm volatile("bar.sync 9, %0;" ::"n"(NC) : "memory");              // every consumer warp's sums are in place
+        if (t < 5) {
+            const double* wp = reinterpret_cast<const double*>(smem_tma + L::WACC_BYTE_OFF);
+            double s = 0.0;
+            if (t < 2) { for (int w = 0; w < TY; ++w) s += wp[(t * TY + w) * 4]; }
+            else { for (int w = 0; w < 2 * TY; ++w) s += wp[w * 4 + t - 1]; }
+            const long long cta = blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z);
+            diag_part[cta * 5 + t] = s;
+        }
     }
 }
 

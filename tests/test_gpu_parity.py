@@ -563,6 +563,59 @@ def test_moving_spheres_against_oracle(oracle_mod, model, dtype, tol, ftol):
 
 
 # ---------------------------------------------------------------------------------------------
+# slab decomposition: several slabs as virtual ranks on the one GPU, ghost planes through lb_export / import_planes
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("world", [1, 2, 3])
+@pytest.mark.parametrize("dtype,tol", [(B.LB_F64, 1e-13), (B.LB_F32, 5e-6)])
+def test_slab_decomposition_virtual_ranks(oracle_mod, world, dtype, tol):
+    from paper_2112_08264_b200 import slab as S
+    nx, ny, nz, steps = 32, 16, 24, 6
+    rr, rb = w.mixture_fields(nx, ny, nz, 41, amp=0.05)
+    u = np.random.default_rng(9).uniform(-0.02, 0.02, (3, nx * ny * nz))
+    o = oracle_mod.Oracle(nx, ny, nz, 0.8, 1.3, 0.9)
+    o.set_fields(rr, rb, *u)
+    o.step(steps)
+    slabs = [S.SlabBox(nx, ny, nz, r, world, 0.8, 1.3, 0.9, dtype=dtype) for r in range(world)]
+    try:
+        for sl in slabs:
+            sl.set_fields(rr, rb, *u)
+        for _ in range(steps):
+            S.ring_exchange_local(slabs)
+            for sl in slabs:
+                sl.step(1)
+        got = np.concatenate([sl.get_populations() for sl in slabs], axis=2)
+    finally:
+        for sl in slabs:
+            sl.close()
+    assert nerr(got, o.get_populations()) < tol
+    # the slabs reproduce the undivided box on the same library bit for bit (same kernel, same values)
+    with B.Box(nx, ny, nz, 0.8, 1.3, 0.9, dtype=dtype) as box:
+        box.set_kernel(B.LB_KERNEL_TWOPASS)
+        box.set_fields(rr, rb, *u)
+        box.step(steps)
+        assert np.array_equal(got, box.get_populations())
+
+
+def test_plane_exchange_argument_checks():
+    import torch
+    with B.Box(32, 8, 6) as box:
+        buf = torch.empty(38 * 2 * 32 * 8, dtype=torch.float64, device="cuda")
+        with pytest.raises(B.LBError) as ei:
+            box.export_planes(0, 2, buf.data_ptr())
+        assert ei.value.code == B.LB_ESTATE
+        box.set_fields(np.ones(32 * 8 * 6), np.ones(32 * 8 * 6))
+        for z0, n in ((-1, 2), (5, 2), (0, 0)):
+            with pytest.raises(B.LBError) as ei:
+                box.export_planes(z0, n, buf.data_ptr())
+            assert ei.value.code == B.LB_EINVAL
+        box.export_planes(4, 2, buf.data_ptr())
+        box.import_planes(0, 2, buf.data_ptr())
+        box.sync()
+        f = box.get_populations()
+        assert np.all(np.isfinite(f))
+
+
+# ---------------------------------------------------------------------------------------------
 # API behaviour on the device
 # ---------------------------------------------------------------------------------------------
 def test_state_and_argument_errors():
@@ -584,9 +637,10 @@ def test_state_and_argument_errors():
         assert box.launch_count() > 0
 
 
+@pytest.mark.parametrize("kernel", [B.LB_KERNEL_TMA, B.LB_KERNEL_HALO], ids=KNAME.get)
 @pytest.mark.parametrize("dtype,tol_m,tol_p", [(B.LB_F64, 1e-13, 1e-10), (B.LB_F32, 1e-5, 1e-3)])
-def test_fused_per_step_diagnostics_match_oracle(oracle_mod, dtype, tol_m, tol_p):
-    """LB_OPT_DIAG: the halo step kernel leaves the mass / momentum sums of the NEW state behind (warp shuffles -> per-CTA
+def test_fused_per_step_diagnostics_match_oracle(oracle_mod, kernel, dtype, tol_m, tol_p):
+    """LB_OPT_DIAG: the TMA / halo step kernel leaves the mass / momentum sums of the NEW state behind (warp shuffles -> per-CTA
     partial -> fixed-order final); lb_get_diagnostics then makes no population pass.  Every one of config 0's 100 steps
     against the oracle's compensated sums (Eq. 6-7), and against the separate-pass diagnostics of the same state."""
     cfg = w.CONFIGS[0]
@@ -594,7 +648,7 @@ def test_fused_per_step_diagnostics_match_oracle(oracle_mod, dtype, tol_m, tol_p
     o = oracle_mod.Oracle(cfg.nx, cfg.ny, cfg.nz, 0.8, 1.3, 0.9)
     o.set_fields(rr, rb)
     with B.Box(cfg.nx, cfg.ny, cfg.nz, 0.8, 1.3, 0.9, dtype=dtype) as box:
-        box.set_kernel(B.LB_KERNEL_HALO)
+        box.set_kernel(kernel)
         box.set_option(B.LB_OPT_DIAG, 1)
         box.set_fields(rr, rb)
         worst_m = worst_p = 0.0
