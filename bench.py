@@ -423,6 +423,23 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
     if args.diag:
         m, p = box.get_diagnostics()            # the sums the last step left behind: no population pass
         diag = {"mass": [float(v) for v in m], "momentum": [float(v) for v in p]}
+    fused = None
+    if not args.diag and mask is None and args.model == "sc" and kname in ("tma", "halo"):
+        # the same K steps once more with the per-step diagnostics fused into the step kernel (LB_OPT_DIAG), for the record
+        box.set_option(B.LB_OPT_DIAG, 1)
+        box.step(3)
+        box.sync()
+        d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        d0.record(stream)
+        box.step(steps)
+        d1.record(stream)
+        d1.synchronize()
+        lq = box.launch_count()
+        m, p = box.get_diagnostics()
+        fused = {"ms_per_step": d0.elapsed_time(d1) / steps, "relative_to_plain": d0.elapsed_time(d1) / ms,
+                 "launches_of_lb_get_diagnostics": box.launch_count() - lq,
+                 "mass": [float(v) for v in m], "momentum": [float(v) for v in p]}
+        box.set_option(B.LB_OPT_DIAG, 0)
 
     # ---- end to end through the C ABI with host buffers ----
     box.sync()
@@ -472,6 +489,8 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
         line["config"]["glups_fluid_nodes_only"] = glups * n_fluid / N      # no computation inside a particle
     if diag:
         line["diagnostics"] = diag
+    if fused:
+        line["diagnostics_fused_run"] = fused
     if cpu_baseline:
         sub = (min(cfg.nx, 128), min(cfg.ny, 128), min(cfg.nz, 64))
         cpu_steps = 12

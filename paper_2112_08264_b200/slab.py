@@ -78,7 +78,9 @@ class SlabBox:
         self.box.step(n)
 
     def get_populations(self):
-        """The rank's own planes [z0, z1): [2][19][nzl][ny][nx]."""
+        """The rank's own planes [z0, z1): [2][19][nzl][ny][nx].  The library keeps the post-collision state and streams when it is
+        read (pull), so the populations of the outermost own planes come out of the ghost planes: exchange once more after the last
+        step before calling this."""
         return self.box.get_populations()[:, :, GHOST:GHOST + self.nzl]
 
     def close(self):

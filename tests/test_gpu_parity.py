@@ -583,6 +583,7 @@ def test_slab_decomposition_virtual_ranks(oracle_mod, world, dtype, tol):
             S.ring_exchange_local(slabs)
             for sl in slabs:
                 sl.step(1)
+        S.ring_exchange_local(slabs)                             # the getter streams out of the ghost planes (pull convention)
         got = np.concatenate([sl.get_populations() for sl in slabs], axis=2)
     finally:
         for sl in slabs:
