@@ -57,8 +57,9 @@ enum { LB_MODEL_SHAN_CHEN = 0, LB_MODEL_COLOUR_GRADIENT = 1 };   /* options of l
  * needs 0 < omega < 2), or G is not finite; NULL (LB_ENOMEM / LB_ECUDA) if device memory or
  * the device is not available; lb_last_error_code() tells which.  Device memory: 2 population
  * buffers of 38*N values; the carried density, 2 x 2 arrays of N values plus tile-edge arrays
- * (about 54 bytes per node in fp64, 27 in fp32, when nx % 32 == 0 and ny % 8 == 0; 32 / 16
- * otherwise); 4 bytes per node of link words; a staging buffer of 40 bytes x min(N, 2^22). */
+ * and, for LB_KERNEL_HALO, 2 x 20/32 N values of x-halo copies (about 70 bytes per node in fp64,
+ * 35 in fp32, when nx % 32 == 0 and ny % 8 == 0; 32 / 16 otherwise); 4 bytes per node of link
+ * words; a staging buffer of 40 bytes x min(N, 2^22). */
 lb_ctx* lb_create(int nx, int ny, int nz, double tau_r, double tau_b, double G);
 
 /* Same, with the population type (LB_F64 / LB_F32: "fp32 populations and fields", all
