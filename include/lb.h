@@ -53,7 +53,7 @@ enum { LB_MODEL_SHAN_CHEN = 0, LB_MODEL_COLOUR_GRADIENT = 1 };   /* options of l
  * Shan-Chen constant G (reading S2: F^k(x) = -G psi^k(x) sum_{i=1..18} w_i psi^kbar(x+c_i) c_i,
  * psi = rho (S3), w_i the lattice weights of PAPER.md:393-398; G > 0 repels).
  * fp64 populations, the library's own stream.
- * NULL (LB_EINVAL) if a dimension is < 1, tau <= 0.5 or not finite (Eq. 2, PAPER.md:84-86,
+ * NULL (LB_EINVAL) if a dimension is < 1, ny or nz > 65535, N >= 2^31, tau <= 0.5 or not finite (Eq. 2, PAPER.md:84-86,
  * needs 0 < omega < 2), or G is not finite; NULL (LB_ENOMEM / LB_ECUDA) if device memory or
  * the device is not available; lb_last_error_code() tells which.  Device memory: 2 population
  * buffers of 38*N values; the carried density, 2 x 2 arrays of N values plus tile-edge arrays

@@ -136,6 +136,21 @@ __device__ __forceinline__ Nbr neighbours(long long n, int nx, int ny, int nz) {
     return b;
 }
 
+// The step-path kernels of the two-pass formulation run one thread block per ROW_BX consecutive x of one (y, z) row: no integer
+// division, the y / z wrap is block-uniform, and consecutive blocks sweep memory in order (a linear sweep moves 6.7-6.9 TB/s on
+// B200 where a march of tile columns moves 6.3: profiles/r2_probes.md).  grid = row_grid(): ny, nz <= 65535 (checked in lb_create).
+constexpr int ROW_BX = 128;
+__device__ __forceinline__ bool row_node(long long& n, Nbr& b, int& x, int& y, int& z, int nx, int ny, int nz) {
+    x = blockIdx.x * ROW_BX + threadIdx.x; y = blockIdx.y; z = blockIdx.z;
+    if (x >= nx) return false;
+    b.o[0][0] = x == 0 ? nx - 1 : x - 1; b.o[0][1] = x; b.o[0][2] = x == nx - 1 ? 0 : x + 1;
+    b.o[1][0] = (long long)nx * (y == 0 ? ny - 1 : y - 1); b.o[1][1] = (long long)nx * y; b.o[1][2] = (long long)nx * (y == ny - 1 ? 0 : y + 1);
+    const long long pl = (long long)nx * ny;
+    b.o[2][0] = pl * (z == 0 ? nz - 1 : z - 1); b.o[2][1] = pl * z; b.o[2][2] = pl * (z == nz - 1 ? 0 : z + 1);
+    n = b.o[2][1] + b.o[1][1] + x;
+    return true;
+}
+
 // the 19 populations of component k arriving at fluid node n: f_i(x) = h_i(x - c_i) (Eq. 5), or
 // h_opp(i)(x) when x - c_i is solid (halfway bounce-back, Eq. 23-24 with u_b = 0).  lk = links[n].
 template <typename T>
@@ -353,15 +368,13 @@ __global__ void __launch_bounds__(256) k_diag_final(const double* __restrict__ p
 // pass 1: rho^k(x,t) = sum_i f_i^k(x,t) (Eq. 6) with f pulled from the h-state.  Solid nodes report 0.
 // Also the initialiser of the one-pass kernel's density arrays (rho_in = the whole sum, edge arrays 0).
 template <typename T>
-__global__ void __launch_bounds__(256) k_density(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
-                                                 int nx, int ny, int nz, T* __restrict__ rho) {
-    const long long N = (long long)nx * ny * nz;
-    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (n >= N) return;
+__global__ void __launch_bounds__(ROW_BX) k_density(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
+                                                    int nx, int ny, int nz, T* __restrict__ rho) {
+    long long n; Nbr b; int x, y, z;
+    if (!row_node(n, b, x, y, z, nx, ny, nz)) return;
     const unsigned lk = links ? links[n] : 0u;
     T r[2] = {T(0), T(0)};
     if (!(lk & SOLID_BIT)) {
-        const Nbr b = neighbours(n, nx, ny, nz);
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
             T fk[Q];
@@ -377,19 +390,17 @@ __global__ void __launch_bounds__(256) k_density(const T* __restrict__ h, const 
 // pass 2: pull (streaming + bounce-back of the previous step), Shan-Chen force, BGK collision with
 // forcing; the post-collision values are written aligned, to be pulled by the next step.
 template <typename T, bool HAS_SOLID>
-__global__ void __launch_bounds__(256) k_collide_pull(const T* __restrict__ h, T* __restrict__ g,
-                                                      const T* __restrict__ rho, const unsigned* __restrict__ links,
-                                                      long long NP, int nx, int ny, int nz,
-                                                      T om_r, T om_b, T G) {
-    const long long N = (long long)nx * ny * nz;
-    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (n >= N) return;
+__global__ void __launch_bounds__(ROW_BX) k_collide_pull(const T* __restrict__ h, T* __restrict__ g,
+                                                         const T* __restrict__ rho, const unsigned* __restrict__ links,
+                                                         long long NP, int nx, int ny, int nz,
+                                                         T om_r, T om_b, T G) {
+    long long n; Nbr b; int x, y, z;
+    if (!row_node(n, b, x, y, z, nx, ny, nz)) return;
     unsigned lk = 0;
     if (HAS_SOLID) {
         lk = links[n];
         if (lk & SOLID_BIT) return;              // no computation inside a particle
     }
-    const Nbr b = neighbours(n, nx, ny, nz);
     T fr[Q], fb[Q];
     pull19<T>(h, NP, 0, n, b, lk, fr);
     pull19<T>(h, NP, 1, n, b, lk, fb);
@@ -424,15 +435,13 @@ __global__ void __launch_bounds__(256) k_collide_pull(const T* __restrict__ h, T
 // ----------------------------------------------------------------------------------------
 // pass 1 of the colour-gradient step: Theta = (rho^1 - rho^2) / (rho^1 + rho^2); 0 on solid and empty nodes (reading C1)
 template <typename T>
-__global__ void __launch_bounds__(256) k_phase_field(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
-                                                     int nx, int ny, int nz, T* __restrict__ theta) {
-    const long long N = (long long)nx * ny * nz;
-    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (n >= N) return;
+__global__ void __launch_bounds__(ROW_BX) k_phase_field(const T* __restrict__ h, const unsigned* __restrict__ links, long long NP,
+                                                        int nx, int ny, int nz, T* __restrict__ theta) {
+    long long n; Nbr b; int x, y, z;
+    if (!row_node(n, b, x, y, z, nx, ny, nz)) return;
     const unsigned lk = links ? links[n] : 0u;
     T th = T(0);
     if (!(lk & SOLID_BIT)) {
-        const Nbr b = neighbours(n, nx, ny, nz);
         T r[2];
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
@@ -465,15 +474,13 @@ template <typename T> __host__ __device__ constexpr T b_pair(int p) { return p <
 //            (Eq. 24) and hands c_i (f*_i + that) to the sphere (Eq. 25-27; readings M1-M4).  The value is stored where the
 //            plain bounce-back finds it: in the node's own slot i of the post-collision state.
 template <typename T, int MODEL, bool MOVING>
-__global__ void __launch_bounds__(256) k_collide_next(const T* __restrict__ h, T* __restrict__ g, const T* __restrict__ aux,
+__global__ void __launch_bounds__(ROW_BX) k_collide_next(const T* __restrict__ h, T* __restrict__ g, const T* __restrict__ aux,
                                                       const unsigned* __restrict__ links, long long NP, int nx, int ny, int nz,
                                                       T om_r, T om_b, T G, T sigma, T beta, T nu_r, T nu_b, SphereView sp) {
-    const long long N = (long long)nx * ny * nz;
-    const long long n = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-    if (n >= N) return;
+    long long n; Nbr b; int x, y, z;
+    if (!row_node(n, b, x, y, z, nx, ny, nz)) return;
     const unsigned lk = links ? links[n] : 0u;
     if (lk & SOLID_BIT) return;
-    const Nbr b = neighbours(n, nx, ny, nz);
     T fr[Q], fb[Q];
     pull19<T>(h, NP, 0, n, b, lk, fr);
     pull19<T>(h, NP, 1, n, b, lk, fb);
@@ -541,7 +548,6 @@ __global__ void __launch_bounds__(256) k_collide_next(const T* __restrict__ h, T
         }
     }
     if (MOVING && (lk & 0x7FFFEu)) {
-        const int x = int(n % nx), y = int((n / nx) % ny), z = int(n / ((long long)nx * ny));
 #pragma unroll
         for (int i = 1; i < Q; ++i) {
             if (!(lk >> i & 1u)) continue;
@@ -574,6 +580,7 @@ __global__ void __launch_bounds__(256) k_collide_next(const T* __restrict__ h, T
 }
 
 inline unsigned blocks_for(long long cnt, int bs) { return unsigned((cnt + bs - 1) / bs); }
+inline dim3 row_grid(const lb_ctx* c) { return dim3(unsigned((c->nx + ROW_BX - 1) / ROW_BX), unsigned(c->ny), unsigned(c->nz)); }
 
 bool onepass_ok(const lb_ctx* c) { return c->nx % OP_TX == 0 && c->ny % OP_TY == 0; }
 
@@ -588,7 +595,7 @@ int ensure_rho(lb_ctx* c) {
         CU(cudaMemsetAsync(c->rho_y[r], 0, size_t(2) * c->s_y * sizeof(T), c->stream));
         CU(cudaMemsetAsync(c->rho_xy[r], 0, size_t(2) * c->s_xy * sizeof(T), c->stream));
     }
-    k_density<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), c->has_solid ? c->links : nullptr,
+    k_density<T><<<row_grid(c), ROW_BX, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), c->has_solid ? c->links : nullptr,
                                                                c->NP, c->nx, c->ny, c->nz, static_cast<T*>(c->rho_in[r]));
     c->launches++;
     CU(cudaGetLastError());
@@ -604,12 +611,12 @@ int step_twopass(lb_ctx* c) {
     const T* h = static_cast<const T*>(c->f[c->cur]);
     T* g = static_cast<T*>(c->f[c->cur ^ 1]);
     const T* rho = static_cast<const T*>(c->rho_in[c->rcur]);
-    const unsigned nb = blocks_for(c->N, 256);
+    const dim3 nb = row_grid(c);
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
     if (c->has_solid)
-        k_collide_pull<T, true><<<nb, 256, 0, c->stream>>>(h, g, rho, c->links, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
+        k_collide_pull<T, true><<<nb, ROW_BX, 0, c->stream>>>(h, g, rho, c->links, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
     else
-        k_collide_pull<T, false><<<nb, 256, 0, c->stream>>>(h, g, rho, nullptr, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
+        k_collide_pull<T, false><<<nb, ROW_BX, 0, c->stream>>>(h, g, rho, nullptr, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G);
     c->launches += 1;
     CU(cudaGetLastError());
     c->cur ^= 1;
@@ -633,9 +640,9 @@ int step_next(lb_ctx* c) {
     T* g = static_cast<T*>(c->f[c->cur ^ 1]);
     T* aux = static_cast<T*>(c->rho_in[c->rcur]);
     const unsigned* lk = c->has_solid ? c->links : nullptr;
-    const unsigned nb = blocks_for(c->N, 256);
-    if (c->model == LB_MODEL_COLOUR_GRADIENT) k_phase_field<T><<<nb, 256, 0, c->stream>>>(h, lk, c->NP, c->nx, c->ny, c->nz, aux);
-    else k_density<T><<<nb, 256, 0, c->stream>>>(h, lk, c->NP, c->nx, c->ny, c->nz, aux);
+    const dim3 nb = row_grid(c);
+    if (c->model == LB_MODEL_COLOUR_GRADIENT) k_phase_field<T><<<nb, ROW_BX, 0, c->stream>>>(h, lk, c->NP, c->nx, c->ny, c->nz, aux);
+    else k_density<T><<<nb, ROW_BX, 0, c->stream>>>(h, lk, c->NP, c->nx, c->ny, c->nz, aux);
     const bool moving = c->nsph > 0;
     SphereView sp = {};
     if (moving) {
@@ -644,7 +651,7 @@ int step_next(lb_ctx* c) {
     }
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G), sg = T(c->sigma), be = T(c->beta);
     const T nu_r = T((c->tau[0] - 0.5) / 3.0), nu_b = T((c->tau[1] - 0.5) / 3.0);
-#define LB_NEXT(MODEL, MOVING) k_collide_next<T, MODEL, MOVING><<<nb, 256, 0, c->stream>>>(h, g, aux, lk, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G, sg, be, nu_r, nu_b, sp)
+#define LB_NEXT(MODEL, MOVING) k_collide_next<T, MODEL, MOVING><<<nb, ROW_BX, 0, c->stream>>>(h, g, aux, lk, c->NP, c->nx, c->ny, c->nz, om_r, om_b, G, sg, be, nu_r, nu_b, sp)
     if (c->model == LB_MODEL_COLOUR_GRADIENT) { if (moving) LB_NEXT(1, true); else LB_NEXT(1, false); }
     else { if (moving) LB_NEXT(0, true); else LB_NEXT(0, false); }
 #undef LB_NEXT
@@ -851,7 +858,7 @@ int ensure_halo_state(lb_ctx* c) {
         CU(cudaMemsetAsync(c->rho_x[r], 0, size_t(2) * c->s_x * sizeof(T), c->stream));
         CU(cudaMemsetAsync(c->rho_y[r], 0, size_t(2) * c->s_y * sizeof(T), c->stream));
         CU(cudaMemsetAsync(c->rho_xy[r], 0, size_t(2) * c->s_xy * sizeof(T), c->stream));
-        k_density<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), nullptr, c->NP, c->nx, c->ny, c->nz,
+        k_density<T><<<row_grid(c), ROW_BX, 0, c->stream>>>(static_cast<const T*>(c->f[c->cur]), nullptr, c->NP, c->nx, c->ny, c->nz,
                                                                    static_cast<T*>(c->rho_in[r]));
         k_edges_from_rho<T><<<blocks_for(c->N, 256), 256, 0, c->stream>>>(static_cast<const T*>(c->rho_in[r]), c->NP, edge_view<T>(c, r),
                                                                           c->nx, c->ny, c->nz, OP_TY);
@@ -976,6 +983,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
     g_err_code = LB_OK;
     if (nx < 1 || ny < 1 || nz < 1) { fail(LB_EINVAL, "box dimensions must be >= 1"); return nullptr; }
     if ((long long)nx * ny * nz > (1ll << 31) - 1) { fail(LB_EINVAL, "box too large (N must fit in 31 bits)"); return nullptr; }
+    if (ny > 65535 || nz > 65535) { fail(LB_EINVAL, "ny and nz must be <= 65535 (one thread block row per (y, z))"); return nullptr; }
     if (!(tau_r > 0.5) || !(tau_b > 0.5) || !std::isfinite(tau_r) || !std::isfinite(tau_b)) {
         fail(LB_EINVAL, "tau must be finite and > 0.5 (0 < omega < 2)"); return nullptr;
     }
