@@ -386,6 +386,8 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
     box.set_kernel(kernel)
     if args.diag:
         box.set_option(B.LB_OPT_DIAG, 1)
+    if args.zc:
+        box.set_option(B.LB_OPT_ZC, args.zc)
     if args.model == "cg":                       # the paper's own two-fluid operator, general two-pass path
         box.set_colour_gradient(args.sigma, args.beta)
     if mask is not None and args.moving_walls:   # prescribed sphere velocities + force / torque per sphere (N2), same path
@@ -470,6 +472,7 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
         "dtype": cfg.dtype, "data": "synthetic",
         "config": {"workload": cfg.name, "box": [cfg.nx, cfg.ny, cfg.nz], "tau": [cfg.tau_r, cfg.tau_b], "G": cfg.G,
                    "solid_spheres": cfg.n_spheres, "kernel": kname, "launches_per_step": launches / steps,
+                   "planes_per_cta": box.get_option(B.LB_OPT_ZC),
                    "l2": f"state {2 * 38 * N * es / 2**30:.1f} GiB vs 126 MB L2" + (", no flush needed" if 2 * 38 * N * es > (1 << 30) else ": L2-resident, launch-bound, reported only"),
                    "parallelism": "replicas only" if world > 1 else "single GPU", "diagnostics_in_step": bool(args.diag),
                    "operator": "colour gradient (sigma %g, beta %g)" % (args.sigma, args.beta) if args.model == "cg" else "Shan-Chen",
@@ -522,6 +525,7 @@ def main():
     ap.add_argument("--f32", action="store_true", help="run the workload in fp32 (e.g. config1 --f32 --model cg: the paper's Table 2 setting)")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
                     help="--gpus N: N independent replicas (north_star: the path does not shard) or ONE box in N z slabs with halo exchange (N3)")
+    ap.add_argument("--zc", type=int, default=0, help="planes per CTA of the one-pass kernels (LB_OPT_ZC); 0 = the library's heuristic")
     ap.add_argument("--diag", action="store_true", help="per-step mass / momentum sums fused into the step kernel (LB_OPT_DIAG)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma", "halo"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -925,8 +925,11 @@ int configure_onepass_kernels() {
     return LB_OK;
 }
 
-// planes per CTA of the TMA kernel: every chunk re-collides 2 extra planes (long chunks), but the grid should fill the
-// SMs (one CTA each) in whole waves, and more waves balance better.  Measured on B200: 256^3 -> 64, 512^3 -> 256.
+// planes per CTA of the TMA kernels: every chunk re-collides 2 extra planes and fills its pipeline (short chunks cost), and the last
+// CTAs of a launch leave SMs idle for about half a CTA's run time (long chunks cost; with solid nodes the CTAs' run times differ and
+// the tail is about a whole one).  time(zc) ~ (zc + 4) * (max(1, waves) + a), waves = CTAs / SMs, a = 0.5 or 1: reproduces the
+// measured order at 256^3 (zc 64: 1.99 ms, 32: 2.04, 128: 2.06), 512^3 (128: 16.08 ms, 64: 16.16, 256: 16.19) and config 4 (32: 2.53 ms,
+// 64: 2.62, 128: 2.75).  lb_set_option(LB_OPT_ZC) overrides.
 int tma_zc(const lb_ctx* c) {
     if (c->zc_req >= 1) {                                             // the kernel wants whole chunks: the largest divisor of nz <= the request
         int zc = c->zc_req < c->nz ? c->zc_req : c->nz;
@@ -936,13 +939,13 @@ int tma_zc(const lb_ctx* c) {
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
     const double tiles = double(c->nx / OP_TX) * (c->ny / OP_TY);
+    const double a = c->has_solid ? 1.0 : 0.5;
     int best = c->nz;
     double best_cost = 1e300;
     for (int zc = 1; zc <= c->nz; ++zc) {
         if (c->nz % zc != 0) continue;
-        const int chunks = c->nz / zc;
-        const double full = std::ceil(tiles * chunks / sms);          // waves of CTAs
-        const double cost = full * (zc + 4) * (1.0 + 0.25 / full);     // planes collided + prologue, per SM; tail imbalance
+        const double waves = tiles * (c->nz / zc) / sms;
+        const double cost = (zc + 4.0) * ((waves > 1.0 ? waves : 1.0) + a);
         if (cost < best_cost) { best_cost = cost; best = zc; }
     }
     return best;
@@ -1157,6 +1160,7 @@ int lb_set_solid_mask(lb_ctx* c, const unsigned char* mask) {
     if (own_tmp) cudaFree(d_mask);
     if (e != cudaSuccess) return fail_cuda(e, "lb_set_solid_mask");
     c->has_solid = any_solid;   // a mask without solid nodes keeps the plain (no link word) kernels
+    c->zc_tma = tma_zc(c);      // the chunk length that balances best depends on it
     if (!c->in_set_spheres) c->nsph = 0;   // a plain mask: every solid at rest
     c->rho_valid = false;
     if (!any_solid) {
