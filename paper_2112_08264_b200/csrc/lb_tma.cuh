@@ -18,18 +18,21 @@
 //     and the lane next to the edge reads that box instead (a different base offset, same instruction).
 //     y: the one warp whose row lies beyond the edge re-loads its 5 affected populations with plain loads.
 //     z wraps in the box coordinate;
-//   * consumers copy the stage into registers and release it at once, so one stage buffers a whole
-//     plane of prefetch; post-collision values are stored straight from registers (aligned, coalesced);
-//   * the two threads of a node exchange rho^k, j^k through shared memory (common velocity, S4) with a
-//     64-thread named barrier per tile row; the y stage of the density gather is double-buffered behind
-//     one split-phase mbarrier per plane (arrive, independent stores, wait); the stage hand-off is
-//     mbarriers only;
+//   * two shared-memory stages: consumers copy their plane into registers and release its stage at once, and the
+//     producer sends for plane j as soon as every consumer warp has left plane j - 2, two iterations before
+//     its use: the loads come straight from DRAM, no L2 prefetch; post-collision values are stored straight
+//     from registers (aligned, coalesced);
+//   * the two threads of a node exchange rho^k, j^k (common velocity, S4) through stage entries they have
+//     already consumed, with a 64-thread named barrier per tile row; the y stage of the density gather is
+//     double-buffered behind one mbarrier per (row, component): a warp waits only for the rows above and
+//     below it (arrive, independent stores, wait); the stage hand-off is mbarriers only;
 //   * three more warps of the producer group assemble the density ring one plane per iteration: every ring
-//     thread owns up to four ring positions for the whole kernel (their piece offsets live in registers),
-//     fetches their pieces with cp.async one iteration ahead and adds them up in the fixed order; a thread
-//     only ever reads landing slots it filled itself, so the ring warps need no barrier among themselves;
-//   * the producer warp group hands registers to the consumers (setmaxnreg): 16 consumer warps at 104
-//     registers, producer group at 64.
+//     thread owns up to four ring positions for the whole kernel (their piece offsets are tabulated in shared
+//     memory), fetches their pieces with cp.async one iteration ahead and adds them up in the fixed order; a
+//     thread only ever reads landing slots it filled itself, so the ring warps need no barrier among themselves;
+//   * the producer warp group hands registers to the consumers (setmaxnreg): 16 consumer warps at 112
+//     registers, producer group at 32;
+//   * optional fused diagnostics (DIAG): per plane a four-value warp reduction of the post-collision moments.
 #pragma once
 #include <cuda.h>
 
@@ -78,11 +81,6 @@ __device__ __forceinline__ void mbar_wait3(void* bar_a, void* bar_b, void* bar_c
 __device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int c0, int c1, int c2, int c3) {
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
                  ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
-}
-// the same box, into L2 only
-__device__ __forceinline__ void tma_prefetch_4d(const CUtensorMap* tm, int c0, int c1, int c2, int c3) {
-    asm volatile("cp.async.bulk.prefetch.tensor.4d.L2.global.tile [%0, {%1, %2, %3, %4}];"
-                 ::"l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
 // plain global stores through a pointer the compiler must treat as opaque (see the running store pointer in the kernel)
 __device__ __forceinline__ void st_global(double* p, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
