@@ -548,25 +548,31 @@ __global__ void __launch_bounds__(ROW_BX) k_collide_next(const T* __restrict__ h
         }
     }
     if (MOVING && (lk & 0x7FFFEu)) {
-#pragma unroll
-        for (int i = 1; i < Q; ++i) {
-            if (!(lk >> i & 1u)) continue;
-            const int p = sp.pid[b.at(dir_cx(i), dir_cy(i), dir_cz(i))];
+        // a loop over the links that exist (few nodes have any, and those few a handful): compact code instead of 18 unrolled copies.
+        // The two values of a link are exchanged with the register arrays through a switch-free select chain on the direction.
+        for (unsigned m = lk & 0x7FFFEu; m; m &= m - 1) {
+            const int i = __ffs(int(m)) - 1;
+            const int cx = dir_cx(i), cy = dir_cy(i), cz = dir_cz(i);
+            const int p = sp.pid[b.at(cx, cy, cz)];
             if (p < 0) continue;
-            double rbv[3] = {x + 0.5 * dir_cx(i) - sp.c[3 * p], y + 0.5 * dir_cy(i) - sp.c[3 * p + 1], z + 0.5 * dir_cz(i) - sp.c[3 * p + 2]};
+            double rbv[3] = {x + 0.5 * cx - sp.c[3 * p], y + 0.5 * cy - sp.c[3 * p + 1], z + 0.5 * cz - sp.c[3 * p + 2]};
             rbv[0] -= nx * floor(rbv[0] / nx + 0.5); rbv[1] -= ny * floor(rbv[1] / ny + 0.5); rbv[2] -= nz * floor(rbv[2] / nz + 0.5);
             const double ub[3] = {sp.v[3 * p] + (rbv[1] * sp.w[3 * p + 2] - rbv[2] * sp.w[3 * p + 1]),      // Eq. 22 as printed
                                   sp.v[3 * p + 1] + (rbv[2] * sp.w[3 * p] - rbv[0] * sp.w[3 * p + 2]),
                                   sp.v[3 * p + 2] + (rbv[0] * sp.w[3 * p + 1] - rbv[1] * sp.w[3 * p])};
             const T wi = i < 7 ? T(1.0 / 18.0) : T(1.0 / 36.0);
-            const T ubi = T(3) * T(ub[0] * dir_cx(i) + ub[1] * dir_cy(i) + ub[2] * dir_cz(i));
-            const T br = fr[i] - T(2) * rr * wi * ubi, bb = fb[i] - T(2) * rb * wi * ubi;            // Eq. 24
-            const double m = (double(fr[i]) + double(br)) + (double(fb[i]) + double(bb));            // momentum handed over along c_i
-            fr[i] = br; fb[i] = bb;
-            const double Fv[3] = {m * dir_cx(i), m * dir_cy(i), m * dir_cz(i)};
-            if (dir_cx(i)) atomicAdd(sp.F + 3 * p, Fv[0]);
-            if (dir_cy(i)) atomicAdd(sp.F + 3 * p + 1, Fv[1]);
-            if (dir_cz(i)) atomicAdd(sp.F + 3 * p + 2, Fv[2]);
+            const T ubi = T(3) * T(ub[0] * cx + ub[1] * cy + ub[2] * cz);
+            T fri = T(0), fbi = T(0);
+#pragma unroll
+            for (int q = 1; q < Q; ++q) if (q == i) { fri = fr[q]; fbi = fb[q]; }
+            const T br = fri - T(2) * rr * wi * ubi, bb = fbi - T(2) * rb * wi * ubi;                  // Eq. 24
+            const double mm = (double(fri) + double(br)) + (double(fbi) + double(bb));                 // momentum handed over along c_i
+#pragma unroll
+            for (int q = 1; q < Q; ++q) if (q == i) { fr[q] = br; fb[q] = bb; }
+            const double Fv[3] = {mm * cx, mm * cy, mm * cz};
+            if (cx) atomicAdd(sp.F + 3 * p, Fv[0]);
+            if (cy) atomicAdd(sp.F + 3 * p + 1, Fv[1]);
+            if (cz) atomicAdd(sp.F + 3 * p + 2, Fv[2]);
             atomicAdd(sp.T + 3 * p, Fv[1] * rbv[2] - Fv[2] * rbv[1]);                                 // Eq. 27 as printed: F x r_b
             atomicAdd(sp.T + 3 * p + 1, Fv[2] * rbv[0] - Fv[0] * rbv[2]);
             atomicAdd(sp.T + 3 * p + 2, Fv[0] * rbv[1] - Fv[1] * rbv[0]);
