@@ -1,7 +1,7 @@
 // lb_halo.cuh -- the fused one-pass time step for boxes without solid nodes: the hot kernel on B200.
 //
 // Same algorithm, state convention (h-state, pull streaming) and warp-specialised structure as lb_tma.cuh, with the two
-// sources of wasted DRAM traffic of that kernel removed (measured there: 692 B/node against 608 algorithmic):
+// sources of wasted DRAM traffic of that kernel removed (measured there: 685-697 B/node against 608 algorithmic):
 //
 //   * x shift without wide boxes.  A TMA box must start 16-byte aligned, so lb_tma.cuh pulls the directions with
 //     c_x != 0 as boxes 16 bytes wider than the tile: 9 sectors per row instead of 8, and the ninth misses in L2
