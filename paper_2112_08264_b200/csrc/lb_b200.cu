@@ -808,12 +808,12 @@ int ensure_diag_buf(lb_ctx* c, long long ncta) {
     return LB_OK;
 }
 
-template <typename T, bool HAS_SOLID, bool DIAG>
+template <typename T, bool HAS_SOLID, bool DIAG, int MODEL = 0>
 int launch_tma(lb_ctx* c) {
-    auto kern = k_step_tma<T, HAS_SOLID, OP_TY, DIAG>;
+    auto kern = k_step_tma<T, HAS_SOLID, OP_TY, DIAG, MODEL>;
     constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
     const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, (c->nz + c->zc_tma - 1) / c->zc_tma);
-    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(c->G);
+    const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(MODEL == 1 ? c->sigma : c->G);
     if (DIAG) {
         const long long ncta = (long long)grid.x * grid.y * grid.z;
         const int rc = ensure_diag_buf(c, ncta);
@@ -823,7 +823,7 @@ int launch_tma(lb_ctx* c) {
     kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                            static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                            rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
-                                                           c->zc_tma, om_r, om_b, G, c->diag_cta);
+                                                           c->zc_tma, om_r, om_b, G, c->diag_cta, T(c->beta));
     c->launches += 1;
     CU(cudaGetLastError());
     return LB_OK;
@@ -833,8 +833,10 @@ template <typename T>
 int step_tma(lb_ctx* c) {
     int rc = ensure_rho<T>(c);
     if (rc != LB_OK) return rc;
-    const bool diag = c->diag_mode && !c->has_solid;        // with bounce-back the walls take momentum: the separate pass does it
-    rc = c->has_solid ? launch_tma<T, true, false>(c) : (diag ? launch_tma<T, false, true>(c) : launch_tma<T, false, false>(c));
+    const bool cg = c->model == LB_MODEL_COLOUR_GRADIENT;   // (effective_kernel sends colour gradient with solids down the two-pass path)
+    const bool diag = c->diag_mode && !c->has_solid && !cg; // with bounce-back the walls take momentum: the separate pass does it
+    rc = cg ? launch_tma<T, false, false, 1>(c)
+            : (c->has_solid ? launch_tma<T, true, false>(c) : (diag ? launch_tma<T, false, true>(c) : launch_tma<T, false, false>(c)));
     if (rc != LB_OK) return rc;
     c->cur ^= 1;
     c->rcur ^= 1;                                           // the kernel wrote rho(t+1)
@@ -926,6 +928,7 @@ int configure_onepass_kernels() {
     CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_tma<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
+    CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_halo<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<false>())));
     CU(cudaFuncSetAttribute(k_step_halo<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<true>())));
     return LB_OK;
@@ -966,8 +969,15 @@ int resolve_kernel(lb_ctx* c, int kind) {
     return kind;
 }
 
+// The later operators run k_collide_next on the two-pass path, except the colour gradient on a box without solids whose kernel
+// choice resolves to the TMA kernel: that one has its own variant of k_step_tma.
+bool next_path(const lb_ctx* c) {
+    if (c->nsph > 0) return true;
+    if (c->model == LB_MODEL_SHAN_CHEN) return false;
+    return c->has_solid || c->kernel != LB_KERNEL_TMA;
+}
 int effective_kernel(const lb_ctx* c) {
-    if (c->model != LB_MODEL_SHAN_CHEN || c->nsph > 0) return LB_KERNEL_TWOPASS;     // the later operators: general two-pass path
+    if (next_path(c)) return LB_KERNEL_TWOPASS;                                      // the later operators: general two-pass path
     return c->kernel == LB_KERNEL_HALO && c->has_solid ? LB_KERNEL_TMA : c->kernel;
 }
 
@@ -1347,7 +1357,7 @@ int lb_step(lb_ctx* c, int nsteps) {
     for (int s = 0; s < nsteps; ++s) {
         int rc;
         const int kern = effective_kernel(c);
-        if (c->model != LB_MODEL_SHAN_CHEN || c->nsph > 0) rc = c->dtype == LB_F64 ? step_next<double>(c) : step_next<float>(c);
+        if (next_path(c)) rc = c->dtype == LB_F64 ? step_next<double>(c) : step_next<float>(c);
         else if (kern == LB_KERNEL_HALO) rc = c->dtype == LB_F64 ? step_halo<double>(c) : step_halo<float>(c);
         else if (kern == LB_KERNEL_TMA) rc = c->dtype == LB_F64 ? step_tma<double>(c) : step_tma<float>(c);
         else if (kern == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);

@@ -99,6 +99,34 @@ __device__ __forceinline__ void collide19_pairs(const T (&f)[Q], T rho, T omc, T
     }
 }
 
+// B_i of the colour-gradient perturbation: -2/9 rest, 1/54 axis, 1/27 diagonal.
+template <typename T> __host__ __device__ constexpr T cg_b_rest() { return T(-2.0 / 9.0); }
+template <typename T> __host__ __device__ constexpr T cg_b_pair(int p) { return p < 3 ? T(1.0 / 54.0) : T(1.0 / 27.0); }
+
+// Colour-gradient collision (readings C1-C6 of DESIGN.md section 3) for ONE component of a node, handed out
+// pair by pair like collide19_pairs.  fs = sum_k f_i^k (the recolouring works on the colour-blind total), rt = rho,
+// x_own = rho^k / rho, (ux, uy, uz) by Eq. 7, om the local relaxation frequency, amp = (A / 2) |grad Theta| with
+// A = (9/4) sigma om (Eq. 17, 19), (gx, gy, gz) = grad Theta, ig2 = 1 / |grad|^2 and ign = 1 / |grad| (0 without a gradient),
+// rcs = +- beta rho^1 rho^2 / rho (Eq. 20: + for the first component, Eq. 21: - for the second).
+template <typename T, typename Rest, typename Pair>
+__device__ __forceinline__ void collide19_cg_pairs(const T (&fs)[Q], T rt, T x_own, T om, T ux, T uy, T uz, T amp, T gx, T gy, T gz,
+                                                    T ig2, T ign, T rcs, Rest rest, Pair pair) {
+    const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
+    const T omc = T(1) - om, amp2 = T(2) * amp;        // both components carry the same perturbation
+    rest(x_own * (omc * fs[0] + om * w_rest<T>() * rt * a0 - amp2 * cg_b_rest<T>()));      // cos(phi_0) = 0: no recolouring term
+#pragma unroll
+    for (int p = 0; p < 9; ++p) {
+        const T cu = cdot<T>(p, ux, uy, uz), cg = cdot<T>(p, gx, gy, gz);
+        const T wr = om * (w_pair<T>(p) * rt);
+        const T s0 = a0 + T(4.5) * cu * cu;
+        const T pert = amp2 * (w_pair<T>(p) * cg * cg * ig2 - cg_b_pair<T>(p));             // Eq. 17: the same for i and opp(i)
+        const T recol = rcs * w_pair<T>(p) * cg * ign * (p < 3 ? T(1) : T(0.70710678118654752440));   // cos(phi_i) = c_i.grad / (|c_i| |grad|)
+        const T f1 = omc * fs[2 * p + 1] + wr * (s0 + T(3) * cu) + pert;
+        const T f2 = omc * fs[2 * p + 2] + wr * (s0 - T(3) * cu) + pert;
+        pair(p, x_own * f1 + recol, x_own * f2 - recol);                                    // Eq. 20-21
+    }
+}
+
 // Eq. 10 for all 19 directions.
 template <typename T>
 __device__ __forceinline__ void equilibrium19(T (&f)[Q], T rho, T ux, T uy, T uz) {

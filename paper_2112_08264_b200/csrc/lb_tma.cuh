@@ -120,8 +120,8 @@ struct TmaLayout {
     static constexpr int SU = RING + 8 * RS;                           // [2][2][2][SUP]  double-buffered z-summed Up, Um per component
     static constexpr int LAND = SU + 8 * SUP;                          // [2][8][96]      landing slots of the ring pieces, per component and ring thread
     static constexpr int EX = LAND + 2 * 8 * 96;                           // [2 TY][2][8]    per tile row and x side: what leaves the tile in x by c_z, and the z pipeline of that export
-    static constexpr int CST = EX + 2 * TY * 2 * 8;                    // {om_r, om_b, G}
-    static constexpr int RTAB = CST + 4;                               // int [9][96]     where the ring threads' pieces live
+    static constexpr int CST = EX + 2 * TY * 2 * 8;                    // {om_r, om_b, G, sigma, beta, 1/nu_r, 1/nu_b}
+    static constexpr int RTAB = CST + 8;                               // int [9][96]     where the ring threads' pieces live
     static constexpr int END = RTAB + (9 * 96 * int(sizeof(int)) + int(sizeof(T)) - 1) / int(sizeof(T));
     static constexpr size_t BAR_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
     // mbarriers: full[2], done[2], rdy, rowpub[2][2 TY]
@@ -141,13 +141,18 @@ struct TmaLayout {
 // behind, one partial per CTA: the post-collision moments sum_i f*_i = rho, sum_i f*_i c_i = (1 - om) j + om rho u' + rho du
 // (Eq. 1, Eq. 10, S5), which streaming in a periodic box only permutes.  Per plane a four-value warp reduction (6 shuffles of
 // doubles) into per-warp shared-memory sums; at the end the 2 TY warp sums in a fixed order.
-template <typename T, bool HAS_SOLID, int TY, bool DIAG = false>
+// MODEL 1 (boxes without solids): the colour-gradient collision instead of Shan-Chen force + BGK.  The ring
+// then holds the phase field Theta of the tile and its frame (the ring warps turn the two assembled densities into Theta), a
+// thread reads BOTH components' populations of its node from the stage (the recolouring works on their sum) and computes its own
+// component's post-collision values: the two threads of a node need no exchange.  G carries sigma, the extra parameter beta.
+template <typename T, bool HAS_SOLID, int TY, bool DIAG = false, int MODEL = 0>
 __global__ void __launch_bounds__(2 * 32 * TY + 128, 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
            const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
-           T om_r, T om_b, T G, double* __restrict__ diag_part = nullptr) {
+           T om_r, T om_b, T G, double* __restrict__ diag_part = nullptr, T beta = T(0)) {
     static_assert(!(DIAG && HAS_SOLID), "the fused sums assume periodic streaming without bounce-back");
+    static_assert(!(MODEL != 0 && (HAS_SOLID || DIAG)), "the colour-gradient variant is built for boxes without solids, without fused sums");
     using L = TmaLayout<T, TY>;
     constexpr int TX = L::TX, NT = L::NT, NC = 2 * NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     static_assert(TY >= 2 && TY <= 8, "one named barrier per tile row (ids 1..TY)");
@@ -182,7 +187,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         mbar_init(rdy, 3);
         for (int b = 0; b < 4 * TY; ++b) mbar_init(rowpub + b, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        sm[L::CST + 0] = om_r; sm[L::CST + 1] = om_b; sm[L::CST + 2] = G;
+        sm[L::CST + 0] = om_r; sm[L::CST + 1] = om_b; sm[L::CST + 2] = G; sm[L::CST + 3] = G; sm[L::CST + 4] = beta;
+        sm[L::CST + 5] = T(3) / (T(1) / om_r - T(0.5)); sm[L::CST + 6] = T(3) / (T(1) / om_b - T(0.5));   // 1 / nu_k, nu_k = c_s^2 (tau_k - 1/2)
     }
     __syncthreads();
 
@@ -276,6 +282,14 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                         if (hxy && mxy == m) v[m] += pxy;
                         if (m < NPOS - 1 || r + m * NR < RS) dst[kk * RS + m * NR] = v[m];
                     }
+                }
+                if (MODEL == 1) {                                           // Theta = (rho^1 - rho^2) / (rho^1 + rho^2), 0 where empty
+#pragma unroll
+                    for (int m = 0; m < NPOS; ++m)
+                        if (m < NPOS - 1 || r + m * NR < RS) {
+                            const T a = dst[m * NR], b = dst[RS + m * NR], sum = a + b;
+                            dst[m * NR] = sum != T(0) ? (a - b) / sum : T(0);
+                        }
                 }
             };
             for (int rp = 0; rp < 2; ++rp) {                                // iteration 0 needs ring planes 0, 1, 2
@@ -402,8 +416,68 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                 if (lk >> dir_opp(i) & 1u) f[i] = __ldg(hn + (long long)(2 * dir_opp(i)) * NP);
         }
 
-        // ---- moments of this component (Eq. 6-7), exchanged with the other component's thread of the same node ----
         T rho = zero, jx = zero, jy = zero, jz = zero;
+        T ux = zero, uy = zero, uz = zero, ex = zero, ey = zero, ez = zero;
+        T cg_rt = zero, cg_x = zero, cg_om = zero, cg_amp = zero, cg_ig2 = zero, cg_ign = zero, cg_rcs = zero;   // MODEL 1 (ex, ey, ez then hold grad Theta)
+        if constexpr (MODEL == 1) {
+            // ---- colour gradient: the other component's populations of this node come out of the same stage; f becomes the colour-blind
+            //      sum, the two densities are summed on the way in the order of moments19 ----
+            const int dk = 1 - 2 * k;
+            const int od0 = dk * NT;
+            const int odp = dk * ((wrap_xlo && lane_lo) ? TY * PADX : TY * W), odm = dk * ((wrap_xhi && lane_hi) ? TY * PADX : TY * W);
+            T fo[Q];
+#pragma unroll
+            for (int i = 0; i < Q; ++i) fo[i] = st[L::slot_off(i) + (dir_cx(i) == 0 ? rd0 + od0 : (dir_cx(i) > 0 ? rdp + odp : rdm + odm))];
+            if (wrap_ylo || wrap_yhi) {
+                const int gy = wrap_ylo ? ny - 1 : 0;
+                const int x = x0 + tx;
+                const int xs[3] = {x == 0 ? nx - 1 : x - 1, x, x == nx - 1 ? 0 : x + 1};
+                const long long zs[3] = {(long long)zt * pl, (long long)zl * pl, (long long)(zl + 1 == nz ? 0 : zl + 1) * pl};
+#pragma unroll
+                for (int i = 1; i < Q; ++i)
+                    if (dir_cy(i) != 0) {
+                        const T v = __ldg(h + (long long)pop_plane(1 - k, i) * NP + zs[1 - dir_cz(i)] + (long long)gy * nx + xs[1 - dir_cx(i)]);
+                        if ((dir_cy(i) > 0 && wrap_ylo) || (dir_cy(i) < 0 && wrap_yhi)) fo[i] = v;
+                    }
+            }
+            T r_own = f[0], r_oth = fo[0];
+            f[0] += fo[0];
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                r_own += f[2 * p + 1] + f[2 * p + 2];
+                r_oth += fo[2 * p + 1] + fo[2 * p + 2];
+                f[2 * p + 1] += fo[2 * p + 1]; f[2 * p + 2] += fo[2 * p + 2];
+            }
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy reads of the stage before the TMA's next writes
+            __syncwarp();
+            if (lane_lo) mbar_arrive(done + sg);        // the producer may refill this stage with the plane after next
+            moments19<T>(f, cg_rt, jx, jy, jz);         // rho and rho u of the mixture (Eq. 7)
+            if (cg_rt != zero) {
+                const T irt = T(1) / cg_rt;
+                ux = jx * irt; uy = jy * irt; uz = jz * irt;
+                cg_x = r_own * irt;
+                const T x_oth = r_oth * irt;
+                const T inv_nu = cg_x * cst[5 + k] + x_oth * cst[6 - k];                            // 1 / nu
+                cg_om = T(2) / (T(6) / inv_nu + T(1));                                             // reading C2
+                // grad Theta = (1 / c_s^2) sum_i w_i Theta(x + c_i) c_i from the ring (reading C1)
+                const T* ring_t = ring + own_r;
+                T d[9];
+#pragma unroll
+                for (int p = 0; p < 9; ++p) {
+                    const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
+                    d[p] = w_pair<T>(p) * (ring_t[sp * 2 * RS + pair_cy(p) * RW + pair_cx(p)] - ring_t[sm_ * 2 * RS - pair_cy(p) * RW - pair_cx(p)]);
+                }
+                ex = T(3) * ((((d[0] + d[3]) + d[4]) + d[5]) + d[6]);
+                ey = T(3) * ((((d[1] + d[3]) - d[4]) + d[7]) + d[8]);
+                ez = T(3) * ((((d[2] + d[5]) - d[6]) + d[7]) - d[8]);
+                const T g2 = ex * ex + ey * ey + ez * ez;
+                if (g2 != zero) { cg_ig2 = T(1) / g2; cg_ign = T(1) / sqrt(g2); }
+                cg_amp = T(0.5) * (T(2.25) * cst[3] * cg_om) * (g2 * cg_ign);                      // (A / 2) |grad|, A = (9/4) sigma omega (Eq. 19)
+                cg_rcs = (k == 0 ? cst[4] : -cst[4]) * cg_x * x_oth * cg_rt;                       // +- beta rho^1 rho^2 / rho
+            }
+        }
+        if constexpr (MODEL == 0) {
+        // ---- moments of this component (Eq. 6-7), exchanged with the other component's thread of the same node ----
         if (fluid) moments19<T>(f, rho, jx, jy, jz);
         else {
 #pragma unroll
@@ -416,7 +490,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             mine[L::slot_off(0)] = rho; mine[L::slot_off(3)] = jx; mine[L::slot_off(4)] = jy; mine[L::slot_off(5)] = jz;
         }
         asm volatile("bar.sync %0, 64;" ::"r"(ty + 1) : "memory");         // the two warps (red, blue) of this tile row
-        T ux = zero, uy = zero, uz = zero, ex = zero, ey = zero, ez = zero;
         {
             const T* other = st + rd0 + (1 - 2 * k) * NT;                  // the partner's entries (other component, same node)
             const T orho = other[L::slot_off(0)], ojx = other[L::slot_off(3)], ojy = other[L::slot_off(4)], ojz = other[L::slot_off(5)];
@@ -454,6 +527,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             const T G_ = cst[2];
             ex = ux - G_ * gx; ey = uy - G_ * gy; ez = uz - G_ * gz;
         }
+        }   // MODEL == 0
         if (DIAG) {
             const double om = 1.0 - double(omc), r_ = store_h ? double(rho) : 0.0;      // the re-collided planes belong to another chunk
             double v0 = r_, v1 = r_ == 0.0 ? 0.0 : double(omc) * double(jx) + r_ * (om * double(ux) + (double(ex) - double(ux)));
@@ -493,9 +567,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             if (do_store) st_global(o, v);
             ptr_step16(o, step16);
         };
-        collide19_pairs<T>(f, rho, omc, ux, uy, uz, ex, ey, ez,
-            [&](T h0) { put(h0); qb0 += h0; },
-            [&](int p, T h1, T h2) {
+        auto on_rest = [&](T h0) { put(h0); qb0 += h0; };
+        auto on_pair = [&](int p, T h1, T h2) {
                 put(h1);
                 put(h2);
                 if (HAS_SOLID) {
@@ -543,7 +616,9 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                         ro.xy[e_xy + zl * psxy] = lane_hi ? h1 : h2;
                     }
                 }
-            });
+            };
+        if constexpr (MODEL == 0) collide19_pairs<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, on_rest, on_pair);
+        else collide19_cg_pairs<T>(f, cg_rt, cg_x, cg_om, ux, uy, uz, cg_amp, ex, ey, ez, cg_ig2, cg_ign, cg_rcs, on_rest, on_pair);
         if (HAS_SOLID) qb0 += bs;
         const T p0 = qa0, pp = qap, pm = qam;               // complete for plane z-1
         qa0 = qb0; qb0 = qc0;
