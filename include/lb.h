@@ -166,7 +166,8 @@ const char* lb_version(void);
 
 /* ---- later operators (the paper's own two-fluid model and its moving walls) -----------------------------------------
  * Colour gradient runs in its own variant of the TMA kernel on boxes without solid nodes that take the 32 x 8 tile
- * (kernel choice AUTO or TMA), everything else (solid nodes, moving walls, other box shapes) on the general two-pass path. */
+ * (kernel choice AUTO or TMA), everything else (solid nodes, moving walls, other box shapes) on the general two-pass path.
+ *
  * Colour-gradient collision (Eq. 8-21): replaces the Shan-Chen force + BGK of lb_step by
  *   Theta = (rho^1 - rho^2) / (rho^1 + rho^2), grad Theta = (1 / c_s^2) sum_i w_i Theta(x + c_i) c_i,
  *   omega = 2 / (6 nu + 1) with 1 / nu = (rho^1 / rho) / nu_1 + (rho^2 / rho) / nu_2, nu_k = c_s^2 (tau_k - 1/2),
