@@ -196,14 +196,16 @@ int lb_get_sphere_forces(lb_ctx* ctx, double* F, double* T);
  * The box of one context can be a z slab of a larger periodic box with two ghost planes on either side: run lb_step on
  * the slab as it is (its own periodic wrap only ever feeds the outermost ghost planes, whose results are thrown away)
  * and, before every step, overwrite the ghost planes with the neighbour slabs' outermost interior planes.  These two
- * calls move whole z planes [z0, z0 + nplanes) of the device state (the 38 population planes in the library's private
- * order and type: 38 * nplanes * nx * ny values of 8 or 4 bytes) to / from a caller-owned DEVICE buffer, on the
- * context's stream, asynchronously: the caller ships the buffer to the neighbour rank (NCCL / peer copy over NVLink)
- * on the same stream or after lb_sync.  An import invalidates the carried density, so the one-pass kernels pay a
- * density pass after it; the two-pass path is unaffected.  paper_2112_08264_b200/slab.py drives this.
- * LB_EINVAL if the range leaves the box, LB_ESTATE before any state was set. */
+ * calls move whole z planes [z0, z0 + nplanes) of the device state to / from a caller-owned DEVICE buffer of
+ * lb_plane_buffer_bytes(ctx, nplanes) bytes (library-private content: the 38 population planes and, when the current
+ * kernel carries the density from step to step (TMA, ONEPASS), that density of the same planes, so that the one-pass
+ * kernels keep running on slabs), on the context's stream, asynchronously: the caller ships the buffer to the
+ * neighbour rank (NCCL / peer copy over NVLink) on the same stream or after lb_sync.  Both ends must be contexts of
+ * the same box cross-section, type and kernel.  paper_2112_08264_b200/slab.py drives this.
+ * LB_EINVAL if the range leaves the box, LB_ESTATE before any state was set; lb_plane_buffer_bytes: -1 on error. */
 int lb_export_planes(lb_ctx* ctx, int z0, int nplanes, void* device_dst);
 int lb_import_planes(lb_ctx* ctx, int z0, int nplanes, const void* device_src);
+long long lb_plane_buffer_bytes(const lb_ctx* ctx, int nplanes);
 
 /* ---- single-fluid calibration path (the paper's case 1, Table 1) --------------
  * One BGK fluid on the same D3Q19 lattice, periodic box, no force, no solids, fused collide +

@@ -30,7 +30,7 @@ SYMBOLS = (
     "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
     "lb_set_option", "lb_get_option", "lb_sync", "lb_last_error", "lb_last_error_code", "lb_version",
     "lb_set_colour_gradient", "lb_set_shan_chen", "lb_set_spheres", "lb_get_sphere_forces",
-    "lb_export_planes", "lb_import_planes",
+    "lb_export_planes", "lb_import_planes", "lb_plane_buffer_bytes",
     "lbs_create", "lbs_destroy", "lbs_set_fields", "lbs_set_populations", "lbs_step", "lbs_get_populations",
     "lbs_get_moments", "lbs_sync", "lbs_launch_count",
 )
@@ -85,6 +85,8 @@ def lib() -> C.CDLL:
     L.lb_get_sphere_forces.argtypes = [C.c_void_p, _dp, _dp]
     L.lb_export_planes.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
     L.lb_import_planes.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+    L.lb_plane_buffer_bytes.restype = C.c_longlong
+    L.lb_plane_buffer_bytes.argtypes = [C.c_void_p, C.c_int]
     L.lbs_create.restype = C.c_void_p
     L.lbs_create.argtypes = [C.c_int, C.c_int, C.c_int, C.c_double, C.c_int, C.c_void_p]
     L.lbs_destroy.restype = None
@@ -285,6 +287,9 @@ class Box:
 
     def export_planes(self, z0, nplanes, device_ptr):
         _chk(lib().lb_export_planes(self.h, z0, nplanes, device_ptr))
+
+    def plane_buffer_bytes(self, nplanes):
+        return int(lib().lb_plane_buffer_bytes(self.h, nplanes))
 
     def import_planes(self, z0, nplanes, device_ptr):
         _chk(lib().lb_import_planes(self.h, z0, nplanes, device_ptr))

@@ -988,6 +988,64 @@ long long round64(long long v) { return (v + 63) / 64 * 64; }
 // the library's error slot (one per thread), shared with lb_single.cu
 void lb_set_error(int code, const char* what) { g_err = what; g_err_code = code; }
 
+// With a kernel that carries the density from step to step (TMA, one-pass) the planes travel WITH their carried density (rho_in
+// and the three edge arrays, all z-major per component): the receiver's ghost planes then hold what the owner computed, the
+// carried density stays valid and the one-pass kernels keep running on slabs.  Other kernels: populations only.
+static bool planes_carry_density(const lb_ctx* c) {
+    const int k = effective_kernel(c);
+    return (k == LB_KERNEL_TMA || k == LB_KERNEL_ONEPASS) && c->rho_x[0] != nullptr;
+}
+static size_t plane_buffer_elems(const lb_ctx* c, int nplanes) {
+    const size_t pl = size_t(c->nx) * c->ny;
+    size_t n = size_t(NPOP) * nplanes * pl;
+    if (planes_carry_density(c)) {
+        const size_t ntx = c->nx / OP_TX, nty = c->ny / OP_TY;
+        n += size_t(2) * nplanes * (pl + nty * ntx * 2 * OP_TY + nty * 2 * c->nx + nty * ntx * 4);
+    }
+    return n;
+}
+template <typename T>
+static int plane_copy_t(lb_ctx* c, int z0, int nplanes, T* dev, bool out) {
+    const size_t pl = size_t(c->nx) * c->ny;
+    auto copy = [&](T* buf, T* arr, size_t comp_stride, size_t per_z, int rows) -> cudaError_t {
+        const size_t width = size_t(nplanes) * per_z * sizeof(T);
+        T* state = arr + size_t(z0) * per_z;
+        return out ? cudaMemcpy2DAsync(buf, width, state, comp_stride * sizeof(T), width, rows, cudaMemcpyDeviceToDevice, c->stream)
+                   : cudaMemcpy2DAsync(state, comp_stride * sizeof(T), buf, width, width, rows, cudaMemcpyDeviceToDevice, c->stream);
+    };
+    const bool dens = planes_carry_density(c);
+    if (dens && out) {                           // what leaves must describe the state
+        const int rc = ensure_rho<T>(c);
+        if (rc != LB_OK) return rc;
+    }
+    T* buf = dev;
+    CU(copy(buf, static_cast<T*>(c->f[c->cur]), size_t(c->NP), pl, NPOP));
+    buf += size_t(NPOP) * nplanes * pl;
+    if (dens) {
+        const size_t ntx = c->nx / OP_TX, nty = c->ny / OP_TY;
+        const size_t psx = nty * ntx * 2 * OP_TY, psy = nty * 2 * size_t(c->nx), psxy = nty * ntx * 4;
+        const int r = c->rcur;
+        CU(copy(buf, static_cast<T*>(c->rho_in[r]), size_t(c->NP), pl, 2));    buf += size_t(2) * nplanes * pl;
+        CU(copy(buf, static_cast<T*>(c->rho_x[r]), size_t(c->s_x), psx, 2));   buf += size_t(2) * nplanes * psx;
+        CU(copy(buf, static_cast<T*>(c->rho_y[r]), size_t(c->s_y), psy, 2));   buf += size_t(2) * nplanes * psy;
+        CU(copy(buf, static_cast<T*>(c->rho_xy[r]), size_t(c->s_xy), psxy, 2));
+    }
+    if (!out) {
+        if (!dens) c->rho_valid = false;         // the carried density no longer describes the state
+        c->hx_valid = false;                     // nor do the x-halo copies and the fused sums
+        c->diag_fresh = false;
+    }
+    return LB_OK;
+}
+static int plane_copy(lb_ctx* c, int z0, int nplanes, void* dev, bool out) {
+    if (!c || !dev) return fail(LB_EINVAL, "NULL argument");
+    if (z0 < 0 || nplanes < 1 || z0 + nplanes > c->nz) return fail(LB_EINVAL, "plane range outside the box (no wrap)");
+    if (!c->have_fields) return fail(LB_ESTATE, "no state to exchange yet");
+    DeviceGuard guard(c->device);
+    return c->dtype == LB_F64 ? plane_copy_t<double>(c, z0, nplanes, static_cast<double*>(dev), out)
+                              : plane_copy_t<float>(c, z0, nplanes, static_cast<float*>(dev), out);
+}
+
 // ----------------------------------------------------------------------------------------
 // C ABI
 // ----------------------------------------------------------------------------------------
@@ -1259,24 +1317,12 @@ int lb_set_spheres(lb_ctx* c, int np, const double* centres, double radius, cons
 }
 
 // ---- slab decomposition: whole z planes of the device state to / from a caller-owned DEVICE buffer ----
-static int plane_copy(lb_ctx* c, int z0, int nplanes, void* dev, bool out) {
-    if (!c || !dev) return fail(LB_EINVAL, "NULL argument");
-    if (z0 < 0 || nplanes < 1 || z0 + nplanes > c->nz) return fail(LB_EINVAL, "plane range outside the box (no wrap)");
-    if (!c->have_fields) return fail(LB_ESTATE, "no state to exchange yet");
-    DeviceGuard guard(c->device);
-    const size_t es = esize(c), pl = size_t(c->nx) * c->ny, width = size_t(nplanes) * pl * es;
-    char* state = static_cast<char*>(c->f[c->cur]) + size_t(z0) * pl * es;
-    if (out) CU(cudaMemcpy2DAsync(dev, width, state, size_t(c->NP) * es, width, NPOP, cudaMemcpyDeviceToDevice, c->stream));
-    else {
-        CU(cudaMemcpy2DAsync(state, size_t(c->NP) * es, dev, width, width, NPOP, cudaMemcpyDeviceToDevice, c->stream));
-        c->rho_valid = false;                    // the carried density / x-halo copies / fused sums no longer describe the state
-        c->hx_valid = false;
-        c->diag_fresh = false;
-    }
-    return LB_OK;
-}
 int lb_export_planes(lb_ctx* c, int z0, int nplanes, void* device_dst) { return plane_copy(c, z0, nplanes, device_dst, true); }
 int lb_import_planes(lb_ctx* c, int z0, int nplanes, const void* device_src) { return plane_copy(c, z0, nplanes, const_cast<void*>(device_src), false); }
+long long lb_plane_buffer_bytes(const lb_ctx* c, int nplanes) {
+    if (!c || nplanes < 1) return -1;
+    return (long long)(plane_buffer_elems(c, nplanes) * esize(c));
+}
 
 int lb_get_sphere_forces(lb_ctx* c, double* F, double* T) {
     if (!c || !F || !T) return fail(LB_EINVAL, "NULL argument");

@@ -36,9 +36,10 @@ def cut_with_ghosts(a, nx, ny, nz, z0, z1):
 
 
 class SlabBox:
-    """One rank's slab on the CUDA library (general two-pass path)."""
+    """One rank's slab on the CUDA library: the default kernel of the box shape (the one-pass TMA kernel where the tile fits; the
+    planes then travel with their carried density), or `kernel`."""
 
-    def __init__(self, nx, ny, nz, rank, world, tau_r=1.0, tau_b=1.0, G=1.2, dtype=None, cuda_stream=None, device=None):
+    def __init__(self, nx, ny, nz, rank, world, tau_r=1.0, tau_b=1.0, G=1.2, dtype=None, cuda_stream=None, device=None, kernel=None):
         import torch
         from . import binding as B
         self.B, self.torch = B, torch
@@ -47,11 +48,18 @@ class SlabBox:
         self.nzl = self.z1 - self.z0
         dtype = B.LB_F64 if dtype is None else dtype
         self.box = B.Box(nx, ny, self.nzl + 2 * GHOST, tau_r, tau_b, G, dtype=dtype, cuda_stream=cuda_stream)
-        self.box.set_kernel(B.LB_KERNEL_TWOPASS)
-        tdt = torch.float64 if dtype == B.LB_F64 else torch.float32
-        n = 38 * GHOST * nx * ny
-        dev = device if device is not None else torch.device("cuda", torch.cuda.current_device())
-        self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = (torch.empty(n, dtype=tdt, device=dev) for _ in range(4))
+        if kernel is not None:
+            self.box.set_kernel(kernel)
+        self.buffer_bytes = None
+        self._tdt = torch.float64 if dtype == B.LB_F64 else torch.float32
+        self._dev = device if device is not None else torch.device("cuda", torch.cuda.current_device())
+
+    def _buffers(self):
+        nbytes = self.box.plane_buffer_bytes(GHOST)                 # depends on the kernel in effect (with / without the carried density)
+        if nbytes != self.buffer_bytes:
+            n = nbytes // (8 if self._tdt == self.torch.float64 else 4)
+            self.send_lo, self.send_hi, self.recv_lo, self.recv_hi = (self.torch.empty(n, dtype=self._tdt, device=self._dev) for _ in range(4))
+            self.buffer_bytes = nbytes
 
     def set_fields(self, rho_r, rho_b, ux=None, uy=None, uz=None):
         """Global fields in; this rank keeps its planes and the ghosts."""
@@ -59,11 +67,13 @@ class SlabBox:
         self.box.set_fields(*a)
 
     def export_low(self):
+        self._buffers()
         self.box.export_planes(GHOST, GHOST, self.send_lo.data_ptr())
         self.box.sync()
         return self.send_lo
 
     def export_high(self):
+        self._buffers()
         self.box.export_planes(self.nzl, GHOST, self.send_hi.data_ptr())
         self.box.sync()
         return self.send_hi
@@ -101,7 +111,7 @@ def ring_exchange_dist(slab, dist, recv_lo=None, recv_hi=None):
     """One rank per process: the same exchange through torch.distributed point-to-point calls (NCCL on GPUs, gloo in the CPU tests).
     `recv_lo` / `recv_hi` default to the slab's own receive buffers."""
     rank, world = dist.get_rank(), dist.get_world_size()
-    lo, hi = slab.export_low(), slab.export_high()
+    lo, hi = slab.export_low(), slab.export_high()          # (the slab's receive buffers exist from here on)
     recv_lo = slab.recv_lo if recv_lo is None else recv_lo
     recv_hi = slab.recv_hi if recv_hi is None else recv_hi
     if world == 1:

@@ -571,9 +571,11 @@ def test_moving_spheres_against_oracle(oracle_mod, model, dtype, tol, ftol):
 # ---------------------------------------------------------------------------------------------
 # slab decomposition: several slabs as virtual ranks on the one GPU, ghost planes through lb_export / import_planes
 # ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", [B.LB_KERNEL_TMA, B.LB_KERNEL_ONEPASS, B.LB_KERNEL_TWOPASS], ids=KNAME.get)
 @pytest.mark.parametrize("world", [1, 2, 3])
 @pytest.mark.parametrize("dtype,tol", [(B.LB_F64, 1e-13), (B.LB_F32, 5e-6)])
-def test_slab_decomposition_virtual_ranks(oracle_mod, world, dtype, tol):
+def test_slab_decomposition_virtual_ranks(oracle_mod, kernel, world, dtype, tol):
+    """With the one-pass kernels the planes travel with their carried density; with the two-pass kernel, populations only."""
     from paper_2112_08264_b200 import slab as S
     nx, ny, nz, steps = 32, 16, 24, 6
     rr, rb = w.mixture_fields(nx, ny, nz, 41, amp=0.05)
@@ -581,7 +583,8 @@ def test_slab_decomposition_virtual_ranks(oracle_mod, world, dtype, tol):
     o = oracle_mod.Oracle(nx, ny, nz, 0.8, 1.3, 0.9)
     o.set_fields(rr, rb, *u)
     o.step(steps)
-    slabs = [S.SlabBox(nx, ny, nz, r, world, 0.8, 1.3, 0.9, dtype=dtype) for r in range(world)]
+    slabs = [S.SlabBox(nx, ny, nz, r, world, 0.8, 1.3, 0.9, dtype=dtype, kernel=kernel) for r in range(world)]
+    assert all(B.lb_kernel_name(sl.box.h) == KNAME[kernel] for sl in slabs)
     try:
         for sl in slabs:
             sl.set_fields(rr, rb, *u)
@@ -597,7 +600,7 @@ def test_slab_decomposition_virtual_ranks(oracle_mod, world, dtype, tol):
     assert nerr(got, o.get_populations()) < tol
     # the slabs reproduce the undivided box on the same library bit for bit (same kernel, same values)
     with B.Box(nx, ny, nz, 0.8, 1.3, 0.9, dtype=dtype) as box:
-        box.set_kernel(B.LB_KERNEL_TWOPASS)
+        box.set_kernel(kernel)
         box.set_fields(rr, rb, *u)
         box.step(steps)
         assert np.array_equal(got, box.get_populations())
@@ -606,7 +609,8 @@ def test_slab_decomposition_virtual_ranks(oracle_mod, world, dtype, tol):
 def test_plane_exchange_argument_checks():
     import torch
     with B.Box(32, 8, 6) as box:
-        buf = torch.empty(38 * 2 * 32 * 8, dtype=torch.float64, device="cuda")
+        assert box.plane_buffer_bytes(2) >= 38 * 2 * 32 * 8 * 8
+        buf = torch.empty(box.plane_buffer_bytes(2) // 8, dtype=torch.float64, device="cuda")
         with pytest.raises(B.LBError) as ei:
             box.export_planes(0, 2, buf.data_ptr())
         assert ei.value.code == B.LB_ESTATE
