@@ -312,7 +312,7 @@ def run_slab(args, cfg, B, torch, dev, rank, local_rank, world):
         dist.init_process_group("nccl", rank=0, world_size=1, device_id=dev)
     dtype = B.LB_F64 if cfg.dtype == "f64" else B.LB_F32
     stream = torch.cuda.current_stream(dev)
-    kernel = {"auto": None, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA, "halo": B.LB_KERNEL_HALO}[args.kernel]
+    kernel = {"auto": None, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA, "halo": B.LB_KERNEL_HALO, "node": B.LB_KERNEL_NODE}[args.kernel]
     sl = S.SlabBox(cfg.nx, cfg.ny, cfg.nz, rank, world, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype, cuda_stream=stream.cuda_stream, device=dev, kernel=kernel)
     rr, rb = cfg.fields()
     sl.set_fields(rr, rb)
@@ -388,7 +388,7 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
 
     stream = torch.cuda.Stream(device=dev)
     box = B.Box(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype, cuda_stream=stream.cuda_stream)
-    kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA, "halo": B.LB_KERNEL_HALO}[args.kernel]
+    kernel = {"auto": B.LB_KERNEL_AUTO, "twopass": B.LB_KERNEL_TWOPASS, "onepass": B.LB_KERNEL_ONEPASS, "tma": B.LB_KERNEL_TMA, "halo": B.LB_KERNEL_HALO, "node": B.LB_KERNEL_NODE}[args.kernel]
     box.set_kernel(kernel)
     if args.diag:
         box.set_option(B.LB_OPT_DIAG, 1)
@@ -533,7 +533,7 @@ def main():
                     help="--gpus N: N independent replicas (north_star: the path does not shard) or ONE box in N z slabs with halo exchange (N3)")
     ap.add_argument("--zc", type=int, default=0, help="planes per CTA of the one-pass kernels (LB_OPT_ZC); 0 = the library's heuristic")
     ap.add_argument("--diag", action="store_true", help="per-step mass / momentum sums fused into the step kernel (LB_OPT_DIAG)")
-    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma", "halo"])
+    ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma", "halo", "node"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     return run_reference(args) if args.impl == "reference" else run_ours(args)

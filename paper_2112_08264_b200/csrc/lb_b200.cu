@@ -22,6 +22,7 @@
 #include "lb_onepass.cuh"
 #include "lb_tma.cuh"
 #include "lb_halo.cuh"
+#include "lb_node.cuh"
 
 using namespace lb;
 
@@ -846,6 +847,28 @@ int step_tma(lb_ctx* c) {
 }
 
 // ----------------------------------------------------------------------------------------
+// one thread per node (lb_node.cuh): same state and arrays as the TMA kernel, boxes without solid nodes
+// ----------------------------------------------------------------------------------------
+template <typename T>
+int step_node(lb_ctx* c) {
+    int rc = ensure_rho<T>(c);
+    if (rc != LB_OK) return rc;
+    auto kern = k_step_node<T, OP_TY>;
+    constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
+    const dim3 grid(c->nx / OP_TX, c->ny / OP_TY, c->nz / c->zc_tma);
+    kern<<<grid, OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
+                                                       static_cast<T*>(c->f[c->cur ^ 1]), rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1),
+                                                       c->NP, c->nx, c->ny, c->nz, c->zc_tma, T(1.0 / c->tau[0]), T(1.0 / c->tau[1]), T(c->G));
+    c->launches += 1;
+    CU(cudaGetLastError());
+    c->cur ^= 1;
+    c->rcur ^= 1;
+    c->hx_valid = false;
+    c->diag_fresh = false;
+    return LB_OK;
+}
+
+// ----------------------------------------------------------------------------------------
 // halo kernel (lb_halo.cuh): boxes without solid nodes
 // ----------------------------------------------------------------------------------------
 template <typename T>
@@ -929,16 +952,16 @@ int configure_onepass_kernels() {
     CU(cudaFuncSetAttribute(k_step_tma<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
+    CU(cudaFuncSetAttribute(k_step_node<T, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_halo<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<false>())));
     CU(cudaFuncSetAttribute(k_step_halo<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<true>())));
     return LB_OK;
 }
 
 // planes per CTA of the TMA kernels: every chunk re-collides 2 extra planes and fills its pipeline (short chunks cost), and the last
-// CTAs of a launch leave SMs idle for about half a CTA's run time (long chunks cost; with solid nodes the CTAs' run times differ and
-// the tail is about a whole one).  time(zc) ~ (zc + 4) * (max(1, waves) + a), waves = CTAs / SMs, a = 0.5 or 1: reproduces the
-// measured order at 256^3 (zc 64: 1.99 ms, 32: 2.04, 128: 2.06), 512^3 (128: 16.08 ms, 64: 16.16, 256: 16.19) and config 4 (32: 2.53 ms,
-// 64: 2.62, 128: 2.75).  lb_set_option(LB_OPT_ZC) overrides.
+// CTAs of a launch leave SMs idle for about half a CTA's run time (long chunks cost).  time(zc) ~ (zc + 4) * (max(1, waves) + 0.5),
+// waves = CTAs / SMs: reproduces the measured order at 256^3 (zc 64: 1.99 ms, 32: 2.04, 128: 2.06), 512^3 (128: 16.08 ms, 64: 16.16,
+// 256: 16.19) and config 4 (64: 2.36 ms, 32: 2.39).  lb_set_option(LB_OPT_ZC) overrides.
 int tma_zc(const lb_ctx* c) {
     if (c->zc_req >= 1) {                                             // the kernel wants whole chunks: the largest divisor of nz <= the request
         int zc = c->zc_req < c->nz ? c->zc_req : c->nz;
@@ -948,7 +971,7 @@ int tma_zc(const lb_ctx* c) {
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
     const double tiles = double(c->nx / OP_TX) * (c->ny / OP_TY);
-    const double a = c->has_solid ? 1.0 : 0.5;
+    const double a = 0.5;
     int best = c->nz;
     double best_cost = 1e300;
     for (int zc = 1; zc <= c->nz; ++zc) {
@@ -965,7 +988,7 @@ int resolve_kernel(lb_ctx* c, int kind) {
     const bool tma_ok = onepass_ok(c) && c->have_tmap;
     if (kind == LB_KERNEL_AUTO) return tma_ok ? LB_KERNEL_TMA : (onepass_ok(c) ? LB_KERNEL_ONEPASS : LB_KERNEL_TWOPASS);
     if (kind == LB_KERNEL_ONEPASS && !onepass_ok(c)) return -1;
-    if ((kind == LB_KERNEL_TMA || kind == LB_KERNEL_HALO) && !tma_ok) return -1;
+    if ((kind == LB_KERNEL_TMA || kind == LB_KERNEL_HALO || kind == LB_KERNEL_NODE) && !tma_ok) return -1;
     return kind;
 }
 
@@ -978,7 +1001,7 @@ bool next_path(const lb_ctx* c) {
 }
 int effective_kernel(const lb_ctx* c) {
     if (next_path(c)) return LB_KERNEL_TWOPASS;                                      // the later operators: general two-pass path
-    return c->kernel == LB_KERNEL_HALO && c->has_solid ? LB_KERNEL_TMA : c->kernel;
+    return (c->kernel == LB_KERNEL_HALO || c->kernel == LB_KERNEL_NODE) && c->has_solid ? LB_KERNEL_TMA : c->kernel;
 }
 
 long long round64(long long v) { return (v + 63) / 64 * 64; }
@@ -993,7 +1016,7 @@ void lb_set_error(int code, const char* what) { g_err = what; g_err_code = code;
 // carried density stays valid and the one-pass kernels keep running on slabs.  Other kernels: populations only.
 static bool planes_carry_density(const lb_ctx* c) {
     const int k = effective_kernel(c);
-    return (k == LB_KERNEL_TMA || k == LB_KERNEL_ONEPASS) && c->rho_x[0] != nullptr;
+    return (k == LB_KERNEL_TMA || k == LB_KERNEL_NODE || k == LB_KERNEL_ONEPASS) && c->rho_x[0] != nullptr;
 }
 static size_t plane_buffer_elems(const lb_ctx* c, int nplanes) {
     const size_t pl = size_t(c->nx) * c->ny;
@@ -1190,7 +1213,7 @@ int lb_set_option(lb_ctx* c, int option, long long value) {
 long long lb_get_option(const lb_ctx* c, int option) {
     if (!c) return -1;
     switch (option) {
-    case LB_OPT_ZC: return (c->kernel == LB_KERNEL_TMA || c->kernel == LB_KERNEL_HALO) ? c->zc_tma : c->zc;
+    case LB_OPT_ZC: return (c->kernel == LB_KERNEL_TMA || c->kernel == LB_KERNEL_HALO || c->kernel == LB_KERNEL_NODE) ? c->zc_tma : c->zc;
     case LB_OPT_DIAG: return c->diag_mode;
     default: return -1;
     }
@@ -1198,7 +1221,8 @@ long long lb_get_option(const lb_ctx* c, int option) {
 
 int lb_set_kernel(lb_ctx* c, int kind) {
     if (!c) return fail(LB_EINVAL, "NULL context");
-    if (kind != LB_KERNEL_AUTO && kind != LB_KERNEL_TWOPASS && kind != LB_KERNEL_ONEPASS && kind != LB_KERNEL_TMA && kind != LB_KERNEL_HALO)
+    if (kind != LB_KERNEL_AUTO && kind != LB_KERNEL_TWOPASS && kind != LB_KERNEL_ONEPASS && kind != LB_KERNEL_TMA && kind != LB_KERNEL_HALO &&
+        kind != LB_KERNEL_NODE)
         return fail(LB_EINVAL, "unknown kernel kind");
     const int r = resolve_kernel(c, kind);
     if (r < 0) return fail(LB_EINVAL, "box shape does not allow this kernel");
@@ -1405,6 +1429,7 @@ int lb_step(lb_ctx* c, int nsteps) {
         const int kern = effective_kernel(c);
         if (next_path(c)) rc = c->dtype == LB_F64 ? step_next<double>(c) : step_next<float>(c);
         else if (kern == LB_KERNEL_HALO) rc = c->dtype == LB_F64 ? step_halo<double>(c) : step_halo<float>(c);
+        else if (kern == LB_KERNEL_NODE) rc = c->dtype == LB_F64 ? step_node<double>(c) : step_node<float>(c);
         else if (kern == LB_KERNEL_TMA) rc = c->dtype == LB_F64 ? step_tma<double>(c) : step_tma<float>(c);
         else if (kern == LB_KERNEL_ONEPASS) rc = c->dtype == LB_F64 ? step_onepass<double>(c) : step_onepass<float>(c);
         else rc = c->dtype == LB_F64 ? step_twopass<double>(c) : step_twopass<float>(c);

@@ -577,19 +577,19 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5), and, pair by pair as the post-collision values
         //      appear: their (aligned, coalesced) stores and the x stage of the density gather
         //      rho(y, t+1) = sum_i h_i(y - c_i): x by warp shuffles, z by register pipelines, y through shared memory.
-        //      A solid node runs the same instructions on zeros (the shuffles need every lane) and stores nothing. ----
+        //      A solid node runs the same instructions on zeros (the shuffles need every lane) and stores those zeros. ----
         // The row sums go straight into the z pipelines of the gather, one per y class (0: c_y = 0, p: c_y = +1, m: c_y = -1):
         // a* = V_+1(z-2) + V_0(z-1) so far, completed by V_-1(z) for plane z-1; b* = V_+1(z-1), taking V_0(z); c* = V_+1(z).
         T qc0 = zero, qcp = zero, qcm = zero;
         T* SUup = SU;                                    // interior: Up summed over z (plane z-1); x frame: Up[c_z = 0] of the virtual column, plane z
         T* SUum = SU + SUP;
         T bs = zero;                                     // bounced-back arrivals of the next step come from this node
-        // Without solids every plane is stored, also the two re-collided ones at the chunk ends: their owner chunk writes the
-        // same bits from the same inputs, and an unconditional store is cheaper than a predicate per store.
-        const bool do_store = !HAS_SOLID || (fluid && store_h);
+        // Every plane is stored, also the two re-collided ones at the chunk ends (their owner chunk writes the same bits from the
+        // same inputs), and with solids every node too: a solid node has collided zeros into zeros, which is what its populations
+        // are in both buffers (S8).  A predicate per store cost 7 % on config 4 (partly written sectors), 3 % without solids.
         T* o = g + (e_own + zl * plu);                   // values arrive in direction order: a running pointer, two planes per step
         auto put = [&](T v) {
-            if (do_store) st_global(o, v);
+            st_global(o, v);
             ptr_step16(o, step16);
         };
         auto on_rest = [&](T h0) { put(h0); qb0 += h0; };
@@ -645,6 +645,9 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         if constexpr (MODEL == 0) collide19_pairs<T>(f, rho, omc, ux, uy, uz, ex, ey, ez, on_rest, on_pair);
         else collide19_cg_pairs<T>(f, cg_rt, cg_x, cg_om, ux, uy, uz, cg_amp, ex, ey, ez, cg_ig2, cg_ign, cg_rcs, on_rest, on_pair);
         if (HAS_SOLID) qb0 += bs;
+        // the collision was the last reader of this plane's link word: fetch the next plane's here, so that its latency
+        // hides behind the rest of the iteration (at the end of the iteration instead: config 4 2.36 -> 2.27 ms)
+        if (HAS_SOLID && it + 1 < niter) lk = __ldg(links + (e_own - unsigned(k * NP)) + (long long)(zl + 1 == nz ? 0 : zl + 1) * pl);
         const T p0 = qa0, pp = qap, pm = qam;               // complete for plane z-1
         qa0 = qb0; qb0 = qc0;
         qap = qbp; qbp = qcp;
@@ -692,7 +695,6 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         }
         zt = zl;
         zl = zl + 1 == nz ? 0 : zl + 1;
-        if (HAS_SOLID && it + 1 < niter) lk = __ldg(links + (e_own - unsigned(k * NP)) + (long long)zl * pl);
     }
     if (DIAG) {
         asm volatile("bar.sync 9, %0;" ::"n"(NC) : "memory");              // every consumer warp's sums are in place

@@ -12,8 +12,8 @@ from paper_2112_08264_b200 import workloads as w
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [B.LB_KERNEL_TWOPASS, B.LB_KERNEL_ONEPASS, B.LB_KERNEL_TMA, B.LB_KERNEL_HALO]
-KNAME = {B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass", B.LB_KERNEL_TMA: "tma", B.LB_KERNEL_HALO: "halo"}
+KERNELS = [B.LB_KERNEL_TWOPASS, B.LB_KERNEL_ONEPASS, B.LB_KERNEL_TMA, B.LB_KERNEL_HALO, B.LB_KERNEL_NODE]
+KNAME = {B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass", B.LB_KERNEL_TMA: "tma", B.LB_KERNEL_HALO: "halo", B.LB_KERNEL_NODE: "node"}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -148,7 +148,7 @@ def test_spheres_64_cube(oracle_mod, kernel):
         fg, fo = box.get_populations(), o.get_populations()
         assert nerr(fg, fo) < 1e-13
         solid = mask.reshape(n, n, n) == 1
-        assert np.all(fg[:, :, solid] == 0.0)                    # exactly zero, never written
+        assert np.all(fg[:, :, solid] == 0.0)                    # S8: exactly zero
         (gmass, _), (omass, _) = box.get_diagnostics(), o.get_diagnostics()
         assert np.abs(gmass / omass - 1).max() < 1e-13
 
@@ -349,7 +349,7 @@ def test_config4_spheres_full_size_sampled_populations(oracle_mod):
             got = f[:, :, z, y, x]
             if M[z, y, x]:
                 n_solid += 1
-                assert np.all(got == 0.0), (x, y, z)             # S8: exactly zero, never written
+                assert np.all(got == 0.0), (x, y, z)             # S8: exactly zero
                 continue
             o = _cutout_oracle(oracle_mod, cfg, R, Bl, M, x, y, z, s, hw)
             want = o.get_populations()[:, :, hw, hw, hw]
