@@ -265,6 +265,7 @@ k_step_halo(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
         }
         // ---- TMA warp: staged plane j goes into stage j & 1 as soon as every consumer warp has left plane j - 2 ----
         const int lane = t - NC;
+        const unsigned long long pol = l2_policy_evict_normal();    // no box is read twice here
         for (int j = 0; j < nstaged; ++j) {
             const int z = z0 - 2 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
@@ -276,9 +277,9 @@ k_step_halo(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
                 for (int i = 0; i < Q; ++i) {
                     const int zq = zw[1 - dir_cz(i)];                       // f_i(x) = h_i(x - c_i)
                     T* slot = stage + s * L::STAGE_ELEMS + L::slot_off(i);
-                    tma_load_4d(slot, &tm_n, full + s, x0, y0 - dir_cy(i), zq, pop_plane(0, i));   // planes q, q + 1: both components
+                    tma_load_4d(slot, &tm_n, full + s, x0, y0 - dir_cy(i), zq, pop_plane(0, i), pol);   // planes q, q + 1: both components
                     if (dir_cx(i) != 0)                                     // the neighbour's column, rows pre-shifted by the writer
-                        tma_load_4d(slot + L::NA, &tm_h, full + s, y0, dir_cx(i) > 0 ? btxm : btxp, zq, 2 * halo_j(i));
+                        tma_load_4d(slot + L::NA, &tm_h, full + s, y0, dir_cx(i) > 0 ? btxm : btxp, zq, 2 * halo_j(i), pol);
                 }
             }
             __syncwarp();

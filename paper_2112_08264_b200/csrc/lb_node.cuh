@@ -170,6 +170,7 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
         // ---- TMA warp: plane j goes into stage j & 1 as soon as every consumer warp has left plane j - 2: a whole iteration
         //      ahead of its use, so the loads come straight from DRAM and need no L2 prefetch ----
         const int lane = t - NC;
+        const unsigned long long pol = l2_policy_evict_last();
         for (int j = 0; j < niter; ++j) {
             const int z = z0 - 1 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
@@ -182,12 +183,12 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
                     const int zq = zw[1 - dir_cz(i)];                       // f_i(x) = h_i(x - c_i)
                     const int q = pop_plane(0, i);                          // the box takes planes q, q + 1: both components
                     T* slot = stage + s * L::STAGE_ELEMS + L::slot_off(i);
-                    if (dir_cx(i) == 0) tma_load_4d(slot, &tm_n, full + s, x0, y0 - dir_cy(i), zq, q);
+                    if (dir_cx(i) == 0) tma_load_4d(slot, &tm_n, full + s, x0, y0 - dir_cy(i), zq, q, pol);
                     else {
-                        tma_load_4d(slot, &tm_w, full + s, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zq, q);
+                        tma_load_4d(slot, &tm_w, full + s, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zq, q, pol);
                         // the column beyond the box edge: columns nx-PADX..nx-1 for c_x > 0, 0..PADX-1 for c_x < 0
-                        if (dir_cx(i) > 0 && wrap_xlo) tma_load_4d(slot + L::XC, &tm_c, full + s, nx - PADX, y0 - dir_cy(i), zq, q);
-                        if (dir_cx(i) < 0 && wrap_xhi) tma_load_4d(slot + L::XC, &tm_c, full + s, 0, y0 - dir_cy(i), zq, q);
+                        if (dir_cx(i) > 0 && wrap_xlo) tma_load_4d(slot + L::XC, &tm_c, full + s, nx - PADX, y0 - dir_cy(i), zq, q, pol);
+                        if (dir_cx(i) < 0 && wrap_xhi) tma_load_4d(slot + L::XC, &tm_c, full + s, 0, y0 - dir_cy(i), zq, q, pol);
                     }
                 }
             }

@@ -78,13 +78,26 @@ __device__ __forceinline__ void mbar_wait3(void* bar_a, void* bar_b, void* bar_c
         "@!PA bra LAB_WAIT3;\n\t}" ::"r"(smem_u32(bar_a)), "r"(smem_u32(bar_b)), "r"(smem_u32(bar_c)), "r"(parity) : "memory");
 }
 // box load: coordinates (x, y, z, plane); x * sizeof(T) must be a multiple of 16 (see header)
-__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int c0, int c1, int c2, int c3) {
-    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
-                 ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+// `pol`: an L2 eviction policy (l2_policy_*)
+__device__ __forceinline__ void tma_load_4d(void* dst, const CUtensorMap* tm, void* bar, int c0, int c1, int c2, int c3, unsigned long long pol) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
+                 ::"r"(smem_u32(dst)), "l"(tm), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(pol) : "memory");
 }
 // plain global stores through a pointer the compiler must treat as opaque (see the running store pointer in the kernel)
-__device__ __forceinline__ void st_global(double* p, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
-__device__ __forceinline__ void st_global(float* p, float v) { asm volatile("st.global.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
+// Streaming (.cs: evict-first in L2): a stored population is next read one time step later, when L2 has long turned over, while
+// the lines the TMA reads are wanted once more by the tile next door (the 16-byte margins of the wide boxes): with the stores
+// evict-first and the loads evict-last more of those second reads hit (512^3 fp64 in bench.py: 16.1 -> 15.9 ms per step).
+__device__ __forceinline__ void st_global(double* p, double v) { asm volatile("st.global.cs.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
+__device__ __forceinline__ void st_global(float* p, float v) { asm volatile("st.global.cs.f32 [%0], %1;" ::"l"(p), "f"(v) : "memory"); }
+__device__ __forceinline__ unsigned long long l2_policy_evict_last() {
+    unsigned long long p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_evict_first() {
+    unsigned long long p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ unsigned long long l2_policy_evict_normal() {
+    unsigned long long p; asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p)); return p;
+}
 // p += step16 * 16 bytes in ONE instruction (IMAD.WIDE.U32 on the otherwise idle fp32/integer-multiply pipe) instead of
 // the add-with-carry pair the compiler emits for a 64-bit pointer increment
 template <typename T>
@@ -311,6 +324,11 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         // ---- TMA warp: plane j goes into stage j & 1 as soon as every consumer warp has left plane j - 2: a whole iteration
         //      ahead of its use, so the loads come straight from DRAM and need no L2 prefetch ----
         const int lane = t - NC;
+#ifndef LB_POL_N
+#define LB_POL_N l2_policy_evict_last
+#define LB_POL_W l2_policy_evict_last
+#endif
+        const unsigned long long pol_n = LB_POL_N(), pol_w = LB_POL_W();
         for (int j = 0; j < niter; ++j) {
             const int z = z0 - 1 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
@@ -323,12 +341,12 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                     const int zq = zw[1 - dir_cz(i)];                       // f_i(x) = h_i(x - c_i)
                     const int q = pop_plane(0, i);                          // the box takes planes q, q + 1: both components
                     T* slot = stage + s * L::STAGE_ELEMS + L::slot_off(i);
-                    if (dir_cx(i) == 0) tma_load_4d(slot, &tm_n, full + s, x0, y0 - dir_cy(i), zq, q);
+                    if (dir_cx(i) == 0) tma_load_4d(slot, &tm_n, full + s, x0, y0 - dir_cy(i), zq, q, pol_n);
                     else {
-                        tma_load_4d(slot, &tm_w, full + s, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zq, q);
+                        tma_load_4d(slot, &tm_w, full + s, dir_cx(i) > 0 ? x0 - PADX : x0, y0 - dir_cy(i), zq, q, pol_w);
                         // the column beyond the box edge: columns nx-PADX..nx-1 for c_x > 0, 0..PADX-1 for c_x < 0
-                        if (dir_cx(i) > 0 && wrap_xlo) tma_load_4d(slot + L::XC, &tm_c, full + s, nx - PADX, y0 - dir_cy(i), zq, q);
-                        if (dir_cx(i) < 0 && wrap_xhi) tma_load_4d(slot + L::XC, &tm_c, full + s, 0, y0 - dir_cy(i), zq, q);
+                        if (dir_cx(i) > 0 && wrap_xlo) tma_load_4d(slot + L::XC, &tm_c, full + s, nx - PADX, y0 - dir_cy(i), zq, q, pol_w);
+                        if (dir_cx(i) < 0 && wrap_xhi) tma_load_4d(slot + L::XC, &tm_c, full + s, 0, y0 - dir_cy(i), zq, q, pol_w);
                     }
                 }
             }
