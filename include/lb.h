@@ -125,13 +125,19 @@ int lb_get_diagnostics(lb_ctx* ctx, double mass[2], double momentum[3]);
  * TMA-staged single pass that reads aligned tiles only (the x neighbour's column comes from
  * x-halo copies) and sums the density of the tile's own nodes from the staged populations
  * instead of carrying it (less DRAM traffic, measured slower; no bounce-back: a box with solid
- * nodes runs LB_KERNEL_TMA instead; ); LB_KERNEL_AUTO (default)
- * = TMA when the box shape allows it (ONEPASS if the driver cannot encode the tensor maps), else
- * TWOPASS: boxes whose sides are not multiples of the 32 x 8 tile run about 1.5 x slower.
- * LB_EINVAL if the box shape does not allow `kind`. */
+ * nodes runs LB_KERNEL_TMA instead); LB_KERNEL_NODE = the TMA-staged single pass with one thread
+ * per node doing both components (LB_KERNEL_TMA: one thread per node and component): a third fewer
+ * instructions for the same bytes, no bounce-back and no fused sums (a box with solid nodes runs
+ * LB_KERNEL_TMA instead); LB_KERNEL_AUTO (default) = the TMA-staged pass when the box shape allows
+ * it (ONEPASS if the driver cannot encode the tensor maps), else TWOPASS: boxes whose sides are not
+ * multiples of the 32 x 8 tile run about 1.5 x slower.  Under AUTO the library picks the thread
+ * mapping itself: LB_KERNEL_NODE for an fp64 Shan-Chen box without solid nodes and without
+ * LB_OPT_DIAG (measured 0.3 - 1 % faster under the board's power cap), LB_KERNEL_TMA otherwise;
+ * lb_get_kernel reports which.  LB_EINVAL if the box shape does not allow `kind`. */
 int lb_set_kernel(lb_ctx* ctx, int kind);
 
-/* The kernel lb_step will use (LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA or LB_KERNEL_HALO; never AUTO); -1 for a NULL context. */
+/* The kernel lb_step will use (LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA, LB_KERNEL_HALO or LB_KERNEL_NODE; never AUTO);
+ * -1 for a NULL context. */
 int lb_get_kernel(const lb_ctx* ctx);
 
 /* Tuning and modes.  LB_OPT_ZC: planes per CTA of the one-pass kernels (each CTA marches over
