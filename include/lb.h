@@ -117,6 +117,19 @@ int lb_get_link_mask(lb_ctx* ctx, unsigned int* links);
  * Accumulated in double for both dtypes.  Synchronises. */
 int lb_get_diagnostics(lb_ctx* ctx, double mass[2], double momentum[3]);
 
+/* lb_get_diagnostics for callers that cannot allocate or synchronise (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same two kernels (per-block partial sums of the moments of Eq. 6-7, then a
+ * fixed-order final pass: deterministic), but the partials live in a static __device__ array of the library instead of
+ * allocated memory, and the five sums {M^r, M^b, P_x, P_y, P_z} go to out_dev, DEVICE memory for 5 doubles owned by the
+ * caller.  Calls no cudaMalloc, cudaFree, memcpy or synchronisation: two launches on the context's stream, the result is
+ * there once the stream reaches that point.  Limit: boxes of at most 2^28 nodes (16384 partials of 16384 nodes each, 640 KB
+ * of device memory that every GPU which loads the library holds until the process exits); a larger box is LB_EINVAL with
+ * a message saying so.  Every call on a device shares that array and finds the last call's contents in it (nothing has to
+ * start at zero: each block overwrites its own partial): calls whose kernels overlap on the GPU (different streams of one
+ * device) race; calls on one stream, or ordered by events, do not.  LB_ESTATE before lb_set_fields / lb_set_populations;
+ * LB_ECUDA if the array's device address could not be obtained when the context was created. */
+int lb_diagnostics_noalloc(lb_ctx* ctx, double* out_dev);
+
 /* Choose the time-step kernel: LB_KERNEL_TWOPASS = density pass + fused collide/stream pass
  * (reads the populations twice per step); LB_KERNEL_ONEPASS = single fused pass that
  * reads and writes every population once per step, populations pulled with per-thread loads;

@@ -27,7 +27,7 @@ LIB_PATH = os.path.join(_HERE, "_lib", "liblb_b200.so")
 SYMBOLS = (
     "lb_create", "lb_create_ex", "lb_destroy", "lb_set_fields", "lb_set_solid_mask",
     "lb_set_populations", "lb_step", "lb_get_populations", "lb_get_moments",
-    "lb_get_link_mask", "lb_get_diagnostics", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
+    "lb_get_link_mask", "lb_get_diagnostics", "lb_diagnostics_noalloc", "lb_set_kernel", "lb_get_kernel", "lb_launch_count",
     "lb_set_option", "lb_get_option", "lb_sync", "lb_last_error", "lb_last_error_code", "lb_version",
     "lb_set_colour_gradient", "lb_set_shan_chen", "lb_set_spheres", "lb_get_sphere_forces",
     "lb_export_planes", "lb_import_planes", "lb_plane_buffer_bytes",
@@ -69,6 +69,7 @@ def lib() -> C.CDLL:
     L.lb_get_moments.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
     L.lb_get_link_mask.argtypes = [C.c_void_p, C.POINTER(C.c_uint)]
     L.lb_get_diagnostics.argtypes = [C.c_void_p, _dp, _dp]
+    L.lb_diagnostics_noalloc.argtypes = [C.c_void_p, C.c_void_p]
     L.lb_set_kernel.argtypes = [C.c_void_p, C.c_int]
     L.lb_launch_count.restype = C.c_longlong
     L.lb_launch_count.argtypes = [C.c_void_p]
@@ -196,6 +197,11 @@ def lb_get_diagnostics(h):
     return mass, mom
 
 
+def lb_diagnostics_noalloc(h, out_dev_ptr):
+    """out_dev_ptr: address of 5 doubles of DEVICE memory (e.g. tensor.data_ptr()); asynchronous on the context's stream."""
+    _chk(lib().lb_diagnostics_noalloc(h, C.c_void_p(out_dev_ptr)))
+
+
 def lb_set_kernel(h, kind):
     _chk(lib().lb_set_kernel(h, kind))
 
@@ -268,6 +274,9 @@ class Box:
 
     def get_diagnostics(self):
         return lb_get_diagnostics(self.h)
+
+    def diagnostics_noalloc(self, out_dev_ptr):
+        lb_diagnostics_noalloc(self.h, out_dev_ptr)
 
     def set_kernel(self, kind):
         lb_set_kernel(self.h, kind)

@@ -14,6 +14,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 
@@ -81,6 +82,7 @@ struct lb_ctx {
     int zc_req;        // lb_set_option(LB_OPT_ZC): planes per CTA of the one-pass kernels, 0 = heuristic
     double* diag_part; // [DIAG_BLOCKS][5]
     double* diag_out;  // [5]
+    double* na_scratch; // device address of g_noalloc_scratch on this context's device (lb_diagnostics_noalloc), nullptr if unknown
     long long launches;
 };
 
@@ -100,6 +102,32 @@ int fail_cuda(cudaError_t e, const char* where) {
     g_err = std::string(where) + ": " + cudaGetErrorString(e);
     g_err_code = e == cudaErrorMemoryAllocation ? LB_ENOMEM : LB_ECUDA;
     return g_err_code;
+}
+
+// ---- lb_diagnostics_noalloc: scratch that exists without any allocation call ----------------------------
+// One partial (5 doubles) per block of k_diag_partial, each block taking NOALLOC_NODES_PER_BLOCK nodes: 16384 blocks x 40 B =
+// 640 KB, held by every GPU that loads the library until the process exits; enough for 2^28 nodes (512^3 = 2^27).
+// In host code `g_noalloc_scratch` is a host-side stand-in, NOT a device address: the address a kernel can use comes from
+// cudaGetSymbolAddress, asked for once per device with that device current (noalloc_scratch_address, called by lb_create_ex).
+constexpr int NOALLOC_MAX_BLOCKS = 16384;
+constexpr long long NOALLOC_NODES_PER_BLOCK = 16384;       // 256 threads x 64 nodes
+}  // namespace
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_MAX_BLOCKS * 5];
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mutex;
+double* g_noalloc_addr[NOALLOC_MAX_DEVICES] = {};
+// device address of the scratch array on `device`, which must be the current device; nullptr (error slot set) on failure
+double* noalloc_scratch_address(int device) {
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) { fail(LB_EINVAL, "lb_diagnostics_noalloc: device ordinal beyond the address table"); return nullptr; }
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_addr[device]) {
+        double* ptr = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_noalloc_scratch);
+        if (e != cudaSuccess) { fail_cuda(e, "cudaGetSymbolAddress(g_noalloc_scratch)"); return nullptr; }
+        g_noalloc_addr[device] = ptr;
+    }
+    return g_noalloc_addr[device];
 }
 
 // every ABI call runs on the context's device, whatever the caller's current device is
@@ -1160,6 +1188,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
         return nullptr;                                  // LB_ECUDA, message set
     }
     c->have_tmap = onepass_ok(c) && make_tmaps(c);
+    c->na_scratch = noalloc_scratch_address(c->device);  // set-up for lb_diagnostics_noalloc; a failure is reported there
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
     c->zc = onepass_zc(c);
@@ -1531,6 +1560,28 @@ int lb_get_diagnostics(lb_ctx* c, double mass[2], double momentum[3]) {
     CU(cudaStreamSynchronize(c->stream));
     mass[0] = h[0]; mass[1] = h[1];
     momentum[0] = h[2]; momentum[1] = h[3]; momentum[2] = h[4];
+    return LB_OK;
+}
+
+// see include/lb.h.  No cudaMalloc / cudaFree / memcpy / synchronisation: two launches on the context's stream.
+int lb_diagnostics_noalloc(lb_ctx* c, double* out_dev) {
+    if (!c || !out_dev) return fail(LB_EINVAL, "NULL argument");
+    const long long nblocks = (c->N + NOALLOC_NODES_PER_BLOCK - 1) / NOALLOC_NODES_PER_BLOCK;
+    if (nblocks > NOALLOC_MAX_BLOCKS)
+        return fail(LB_EINVAL, "lb_diagnostics_noalloc: the box has more than 2^28 nodes, beyond the static scratch (16384 partials); use lb_get_diagnostics");
+    if (!c->have_fields) return fail(LB_ESTATE, "lb_diagnostics_noalloc before lb_set_fields / lb_set_populations");
+    if (!c->na_scratch) return fail(LB_ECUDA, "lb_diagnostics_noalloc: the address of the static scratch could not be obtained when the context was created");
+    DeviceGuard guard(c->device);
+    const unsigned* lk = c->has_solid ? c->links : nullptr;
+    // every block overwrites its own partial and k_diag_final reads the first nblocks only: nothing has to start at zero,
+    // whatever an earlier call (another context, another size) left in the array
+    if (c->dtype == LB_F64)
+        k_diag_partial<double><<<int(nblocks), 256, 0, c->stream>>>(static_cast<const double*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, c->na_scratch);
+    else
+        k_diag_partial<float><<<int(nblocks), 256, 0, c->stream>>>(static_cast<const float*>(c->f[c->cur]), lk, c->NP, c->nx, c->ny, c->nz, c->na_scratch);
+    k_diag_final<<<1, 256, 0, c->stream>>>(c->na_scratch, int(nblocks), out_dev);
+    c->launches += 2;
+    CU(cudaGetLastError());
     return LB_OK;
 }
 
