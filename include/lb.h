@@ -154,7 +154,9 @@ int lb_set_kernel(lb_ctx* ctx, int kind);
 int lb_get_kernel(const lb_ctx* ctx);
 
 /* Tuning and modes.  LB_OPT_ZC: planes per CTA of the one-pass kernels (each CTA marches over
- * value z planes and re-collides one more at either end); 0 = the library's heuristic (default).
+ * value z planes and re-collides one more at either end); 0 = the library's heuristic (default),
+ * which also cuts the last few tile rows into one chunk more so that the TMA-staged kernels' CTA count
+ * is a multiple of the SM count (an explicit value keeps every chunk at exactly `value` planes).
  * LB_OPT_DIAG (0 / 1, default 0): per-step diagnostics fused into the step: with LB_KERNEL_TMA and
  * LB_KERNEL_HALO on a box without solid nodes, every lb_step leaves the per-component mass and the
  * total momentum of the NEW state behind (warp-shuffle reductions, one partial per CTA, added in

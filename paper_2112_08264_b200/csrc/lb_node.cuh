@@ -19,7 +19,7 @@ template <typename T, int TY>
 __global__ void __launch_bounds__(32 * TY + 128, 1)
 k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
             const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g,
-            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G) {
+            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G, int row_split = 1 << 30) {
     using L = TmaLayout<T, TY>;
     constexpr int TX = L::TX, NT = L::NT, NC = NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     constexpr bool HAS_SOLID = false;
@@ -45,13 +45,19 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
     const int ntx = nx / TX, nty = ny / TY;
     const int btx = blockIdx.x, bty = blockIdx.y;
     const int x0 = btx * TX, y0 = bty * TY;
-    const int z0 = blockIdx.z * zc;
-    const int niter = zc + 2;
+    int z0, niter_cta;
+    if (!chunk_range(bty, row_split, nz, zc, z0, niter_cta)) return;
+    // The iteration count differs between CTAs: it lives in shared memory and is re-read where it is used (a register held across
+    // the plane loop costs the consumers a spill: +9 local loads per plane, 3.5 % of the step).
+    int* const niter_slot = reinterpret_cast<int*>(sm + L::CST + 8);
+    auto NITER = [&]() { return *reinterpret_cast<volatile const int*>(niter_slot); };
+    auto Z0 = [&]() { return *reinterpret_cast<volatile const int*>(niter_slot + 1); };   // likewise, for the producer group (32 registers)
     const long long pl = (long long)nx * ny;
     const bool wrap_xlo = btx == 0, wrap_xhi = btx == ntx - 1;
     auto wrapz = [&](int p) { p %= nz; return p < 0 ? p + nz : p; };
 
     if (t == 0) {
+        niter_slot[0] = niter_cta; niter_slot[1] = z0;
         for (int s = 0; s < 2; ++s) { mbar_init(full + s, 1); mbar_init(done + s, TY); }
         mbar_init(rdy, 3);
         for (int b = 0; b < 4 * TY; ++b) mbar_init(rowpub + b, 1);
@@ -112,7 +118,7 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
             T* land = sm + L::LAND + r;                                    // [2][8][96]: per component the 4 `in`, x, y, y, xy landing slots of thread r
             // ask for the pieces of ring plane rp (= box plane z0 - 2 + rp): asynchronous, no registers in flight
             auto ring_fetch = [&](int rp) {
-                const unsigned zp = unsigned(wrapz(z0 - 2 + rp));
+                const unsigned zp = unsigned(wrapz(Z0() - 2 + rp));
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                     const int off = rt[j * NR];
@@ -156,14 +162,14 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
                 ring_assemble(rp);
             }
             ring_fetch(2);
-            for (int j = 0; j < niter; ++j) {
+            for (int j = 0; j < NITER(); ++j) {
                 // ring plane j+2 (the z+1 neighbour plane of iteration j): its slot held plane j-2, last read in iteration
                 // j-2, which every consumer warp had left when it arrived on done(j-1)
                 if (j > 0) mbar_wait(done + ((j - 1) & 1), ((j - 1) >> 1) & 1);
                 ring_assemble(j + 2);
                 __syncwarp();
                 if ((r & 31) == 0) mbar_arrive(rdy);
-                if (j + 3 <= niter + 1) ring_fetch(j + 3);
+                if (j + 3 <= NITER() + 1) ring_fetch(j + 3);
             }
             return;
         }
@@ -171,8 +177,8 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
         //      ahead of its use, so the loads come straight from DRAM and need no L2 prefetch ----
         const int lane = t - NC;
         const unsigned long long pol = l2_policy_evict_last();
-        for (int j = 0; j < niter; ++j) {
-            const int z = z0 - 1 + j;
+        for (int j = 0; j < NITER(); ++j) {
+            const int z = Z0() - 1 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
             if (lane == 0) {
                 const int s = j & 1;
@@ -227,8 +233,8 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
     int zl = wrapz(z0 - 1), zt = wrapz(z0 - 2);
 
 #pragma unroll 1
-    for (int it = 0; it < niter; ++it) {
-        const bool store_h = it >= 1 && it <= niter - 2;
+    for (int it = 0; it < NITER(); ++it) {
+        const bool store_h = it >= 1 && it <= NITER() - 2;
         const bool store_rho = it >= 2;
         const int s0 = (it + 1) & 3;
         const int sg = it & 1;

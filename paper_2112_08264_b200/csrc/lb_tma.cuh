@@ -134,7 +134,7 @@ struct TmaLayout {
     static constexpr int LAND = SU + 8 * SUP;                          // [2][8][96]      landing slots of the ring pieces, per component and ring thread
     static constexpr int EX = LAND + 2 * 8 * 96;                           // [2 TY][2][8]    per tile row and x side: what leaves the tile in x by c_z, and the z pipeline of that export
     static constexpr int CST = EX + 2 * TY * 2 * 8;                    // {om_r, om_b, G, sigma, beta, 1/nu_r, 1/nu_b}
-    static constexpr int RTAB = CST + 8;                               // int [9][96]     where the ring threads' pieces live
+    static constexpr int RTAB = CST + 10;                              // CST + 8: int {iterations of this CTA, its first plane}                               // int [9][96]     where the ring threads' pieces live
     static constexpr int END = RTAB + (9 * 96 * int(sizeof(int)) + int(sizeof(T)) - 1) / int(sizeof(T));
     static constexpr size_t BAR_BYTE_OFF = (size_t(END) * sizeof(T) + 15) / 16 * 16;
     // mbarriers: full[2], done[2], rdy, rowpub[2][2 TY]
@@ -145,6 +145,25 @@ struct TmaLayout {
 };
 
 
+
+// ---- which z chunk a CTA takes ---------------------------------------------------------------------------------
+// Grid (ntx, nty, chunks).  Tile rows bty < row_split are cut into nz / zc chunks of zc planes; the rows from row_split on (the
+// host picks how many, so that the number of working CTAs is a multiple of the SM count: one CTA per SM, and a last wave that
+// leaves a third of the SMs idle costs more than it looks) into one chunk more, of nz / (nz / zc + 1) planes or one more; the
+// grid then has one more z layer, in which only those rows work.  Returns false for a CTA without work; niter = planes + 2.
+__device__ __forceinline__ bool chunk_range(int bty, int row_split, int nz, int zc, int& z0, int& niter) {
+    const int c = blockIdx.z;
+    if (bty < row_split) {
+        if (c * zc >= nz) return false;
+        z0 = c * zc;
+        niter = zc + 2;
+    } else {
+        const int m = nz / zc + 1;
+        z0 = c * nz / m;
+        niter = (c + 1) * nz / m - z0 + 2;
+    }
+    return true;
+}
 
 // ---- the kernel ------------------------------------------------------------------------------------------
 // Threads: 2*NT consumers (component k = t / NT, node (tx, ty) = ((t % NT) % 32, (t % NT) / 32): one warp per
@@ -163,7 +182,7 @@ __global__ void __launch_bounds__(2 * 32 * TY + 128, 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
            const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
-           T om_r, T om_b, T G, double* __restrict__ diag_part = nullptr, T beta = T(0)) {
+           T om_r, T om_b, T G, double* __restrict__ diag_part = nullptr, T beta = T(0), int row_split = 1 << 30) {
     static_assert(!(DIAG && HAS_SOLID), "the fused sums assume periodic streaming without bounce-back");
     static_assert(!(MODEL != 0 && (HAS_SOLID || DIAG)), "the colour-gradient variant is built for boxes without solids, without fused sums");
     using L = TmaLayout<T, TY>;
@@ -188,14 +207,20 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const int ntx = nx / TX, nty = ny / TY;
     const int btx = blockIdx.x, bty = blockIdx.y;
     const int x0 = btx * TX, y0 = bty * TY;
-    const int z0 = blockIdx.z * zc;           // the host guarantees nz % zc == 0: every chunk has zc planes
-    const int niter = zc + 2;                 // planes z0-1 .. z0+zc; the first and the last are re-collided only
+    int z0, niter_cta;                        // planes z0-1 .. z0+niter-2; the first and the last are re-collided only
+    if (!chunk_range(bty, row_split, nz, zc, z0, niter_cta)) return;   // (the host guarantees nz % zc == 0)
+    // The iteration count differs between CTAs: it lives in shared memory and is re-read where it is used (a register held across
+    // the plane loop costs the consumers a spill: +9 local loads per plane, 3.5 % of the step).
+    int* const niter_slot = reinterpret_cast<int*>(sm + L::CST + 8);
+    auto NITER = [&]() { return *reinterpret_cast<volatile const int*>(niter_slot); };
+    auto Z0 = [&]() { return *reinterpret_cast<volatile const int*>(niter_slot + 1); };   // likewise, for the producer group (32 registers)
     const long long pl = (long long)nx * ny;
     const bool wrap_xlo = btx == 0, wrap_xhi = btx == ntx - 1;             // the TMA zero-fills outside the box: x wraps with an
                                                                            // extra box per direction, y with consumer loads
     auto wrapz = [&](int p) { p %= nz; return p < 0 ? p + nz : p; };
 
     if (t == 0) {
+        niter_slot[0] = niter_cta; niter_slot[1] = z0;
         for (int s = 0; s < 2; ++s) { mbar_init(full + s, 1); mbar_init(done + s, 2 * TY); }
         mbar_init(rdy, 3);
         for (int b = 0; b < 4 * TY; ++b) mbar_init(rowpub + b, 1);
@@ -258,7 +283,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
             T* land = sm + L::LAND + r;                                    // [2][8][96]: per component the 4 `in`, x, y, y, xy landing slots of thread r
             // ask for the pieces of ring plane rp (= box plane z0 - 2 + rp): asynchronous, no registers in flight
             auto ring_fetch = [&](int rp) {
-                const unsigned zp = unsigned(wrapz(z0 - 2 + rp));
+                const unsigned zp = unsigned(wrapz(Z0() - 2 + rp));
 #pragma unroll
                 for (int j = 0; j < 8; ++j) {
                     const int off = rt[j * NR];
@@ -310,14 +335,14 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
                 ring_assemble(rp);
             }
             ring_fetch(2);
-            for (int j = 0; j < niter; ++j) {
+            for (int j = 0; j < NITER(); ++j) {
                 // ring plane j+2 (the z+1 neighbour plane of iteration j): its slot held plane j-2, last read in iteration
                 // j-2, which every consumer warp had left when it arrived on done(j-1)
                 if (j > 0) mbar_wait(done + ((j - 1) & 1), ((j - 1) >> 1) & 1);
                 ring_assemble(j + 2);
                 __syncwarp();
                 if ((r & 31) == 0) mbar_arrive(rdy);
-                if (j + 3 <= niter + 1) ring_fetch(j + 3);
+                if (j + 3 <= NITER() + 1) ring_fetch(j + 3);
             }
             return;
         }
@@ -329,8 +354,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
 #define LB_POL_W l2_policy_evict_last
 #endif
         const unsigned long long pol_n = LB_POL_N(), pol_w = LB_POL_W();
-        for (int j = 0; j < niter; ++j) {
-            const int z = z0 - 1 + j;
+        for (int j = 0; j < NITER(); ++j) {
+            const int z = Z0() - 1 + j;
             const int zw[3] = {wrapz(z - 1), wrapz(z), wrapz(z + 1)};
             if (lane == 0) {
                 const int s = j & 1;
@@ -398,8 +423,8 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     if (HAS_SOLID) lk = __ldg(links + (e_own - unsigned(k * NP)) + (long long)zl * pl);
 
 #pragma unroll 1
-    for (int it = 0; it < niter; ++it) {
-        const bool store_h = it >= 1 && it <= niter - 2;
+    for (int it = 0; it < NITER(); ++it) {
+        const bool store_h = it >= 1 && it <= NITER() - 2;
         const bool store_rho = it >= 2;                 // target plane z-1 lies in [z0, z1)
         const int s0 = (it + 1) & 3;                    // ring slot of plane z
         const bool fluid = !HAS_SOLID || !(lk & OP_SOLID_BIT);   // nothing happens inside a particle
@@ -665,7 +690,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
         if (HAS_SOLID) qb0 += bs;
         // the collision was the last reader of this plane's link word: fetch the next plane's here, so that its latency
         // hides behind the rest of the iteration (at the end of the iteration instead: config 4 2.36 -> 2.27 ms)
-        if (HAS_SOLID && it + 1 < niter) lk = __ldg(links + (e_own - unsigned(k * NP)) + (long long)(zl + 1 == nz ? 0 : zl + 1) * pl);
+        if (HAS_SOLID && it + 1 < NITER()) lk = __ldg(links + (e_own - unsigned(k * NP)) + (long long)(zl + 1 == nz ? 0 : zl + 1) * pl);
         const T p0 = qa0, pp = qap, pm = qam;               // complete for plane z-1
         qa0 = qb0; qb0 = qc0;
         qap = qbp; qbp = qcp;
