@@ -1010,6 +1010,10 @@ int configure_onepass_kernels() {
 // CTAs of a launch leave SMs idle for about half a CTA's run time (long chunks cost).  time(zc) ~ (zc + 4) * (max(1, waves) + 0.5),
 // waves = CTAs / SMs: reproduces the measured order at 256^3 (zc 64: 1.99 ms, 32: 2.04, 128: 2.06), 512^3 (128: 16.08 ms, 64: 16.16,
 // 256: 16.19) and config 4 (64: 2.36 ms, 32: 2.39).  lb_set_option(LB_OPT_ZC) overrides.
+// k_step_node (with the CTA count padded to whole waves, tma_grid) is faster on shorter chunks than the model says: 512^3 64 planes
+// 15.42 ms, 128: 15.79, 32: 15.76, 256: 16.04; 256^3 64 / 32: 1.97, 128: 2.02 (k_step_tma: 512^3 128: 15.70, 64: 15.80; fp32 128: 9.25,
+// 64: 9.36): for it the candidates are the divisors of nz between 16 and 64, when there are any.
+int effective_kernel(const lb_ctx* c);
 int tma_zc(const lb_ctx* c) {
     if (c->zc_req >= 1) {                                             // the kernel wants whole chunks: the largest divisor of nz <= the request
         int zc = c->zc_req < c->nz ? c->zc_req : c->nz;
@@ -1022,8 +1026,11 @@ int tma_zc(const lb_ctx* c) {
     const double a = 0.5;
     int best = c->nz;
     double best_cost = 1e300;
+    bool short_only = false;
+    if (effective_kernel(c) == LB_KERNEL_NODE && tiles * c->nz / 64.0 >= 2.0 * sms)      // (small boxes: the model below)
+        for (int zc = 16; zc <= 64 && zc <= c->nz; ++zc) short_only = short_only || c->nz % zc == 0;
     for (int zc = 1; zc <= c->nz; ++zc) {
-        if (c->nz % zc != 0) continue;
+        if (c->nz % zc != 0 || (short_only && (zc < 16 || zc > 64))) continue;
         const double waves = tiles * (c->nz / zc) / sms;
         const double cost = (zc + 4.0) * ((waves > 1.0 ? waves : 1.0) + a);
         if (cost < best_cost) { best_cost = cost; best = zc; }
@@ -1270,7 +1277,7 @@ int lb_set_option(lb_ctx* c, int option, long long value) {
 long long lb_get_option(const lb_ctx* c, int option) {
     if (!c) return -1;
     switch (option) {
-    case LB_OPT_ZC: return (c->kernel == LB_KERNEL_TMA || c->kernel == LB_KERNEL_HALO || c->kernel == LB_KERNEL_NODE) ? c->zc_tma : c->zc;
+    case LB_OPT_ZC: return (c->kernel == LB_KERNEL_TMA || c->kernel == LB_KERNEL_HALO || c->kernel == LB_KERNEL_NODE) ? tma_zc(c) : c->zc;
     case LB_OPT_DIAG: return c->diag_mode;
     default: return -1;
     }
@@ -1481,6 +1488,7 @@ int lb_step(lb_ctx* c, int nsteps) {
     DeviceGuard guard(c->device);
     if (nsteps < 0) return fail(LB_EINVAL, "nsteps must be >= 0");
     if (!c->have_fields) return fail(LB_ESTATE, "lb_step before lb_set_fields / lb_set_populations");
+    c->zc_tma = tma_zc(c);                    // depends on which kernel the state of the context selects
     for (int s = 0; s < nsteps; ++s) {
         int rc;
         const int kern = effective_kernel(c);
