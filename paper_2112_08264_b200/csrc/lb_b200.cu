@@ -829,20 +829,19 @@ bool make_tmaps(lb_ctx* c) {
 }
 
 // Grid of k_step_tma / k_step_node (chunk_range in lb_tma.cuh): nz / zc_tma chunks per tile column; when the planes per CTA were
-// left to the library (and the kernel keeps no per-CTA sums), the last rows of tile columns, from row_split on, are cut into one
-// chunk more so that the number of working CTAs comes as close to a multiple of the SM count as whole tile rows allow.
-dim3 tma_grid(const lb_ctx* c, bool allow_balance, int& row_split) {
+// left to the library (and the kernel keeps no per-CTA sums), the last tile columns, from col_split on, are cut into one chunk
+// more so that the number of working CTAs is a multiple of the SM count.
+dim3 tma_grid(const lb_ctx* c, bool allow_balance, int& col_split) {
     const int ntx = c->nx / OP_TX, nty = c->ny / OP_TY, nchunk = c->nz / c->zc_tma;
-    row_split = nty;
+    col_split = ntx * nty;
     if (allow_balance && c->zc_req == 0 && c->balance) {
         int sms = 148;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, c->device);
         const long long total = (long long)ntx * nty * nchunk;
-        const int more = int((sms - total % sms) % sms);               // CTAs missing to the next multiple
-        const int rows = (more + ntx / 2) / ntx;                       // one more CTA per tile column of these rows
-        if (total > sms && rows >= 1 && rows < nty && c->nz / (nchunk + 1) >= 8) row_split = nty - rows;
+        const int more = int((sms - total % sms) % sms);               // CTAs missing to the next multiple: one more per tile column
+        if (total > sms && more >= 1 && more < ntx * nty && c->nz / (nchunk + 1) >= 8) col_split = ntx * nty - more;
     }
-    return dim3(ntx, nty, row_split < nty ? nchunk + 1 : nchunk);
+    return dim3(ntx, nty, col_split < ntx * nty ? nchunk + 1 : nchunk);
 }
 
 int ensure_diag_buf(lb_ctx* c, long long ncta) {
@@ -859,8 +858,8 @@ template <typename T, bool HAS_SOLID, bool DIAG, int MODEL = 0>
 int launch_tma(lb_ctx* c) {
     auto kern = k_step_tma<T, HAS_SOLID, OP_TY, DIAG, MODEL>;
     constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
-    int row_split;
-    const dim3 grid(tma_grid(c, !DIAG, row_split));
+    int col_split;
+    const dim3 grid(tma_grid(c, !DIAG, col_split));
     const T om_r = T(1.0 / c->tau[0]), om_b = T(1.0 / c->tau[1]), G = T(MODEL == 1 ? c->sigma : c->G);
     if (DIAG) {
         const long long ncta = (long long)grid.x * grid.y * grid.z;
@@ -871,7 +870,7 @@ int launch_tma(lb_ctx* c) {
     kern<<<grid, 2 * OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                            static_cast<T*>(c->f[c->cur ^ 1]), HAS_SOLID ? c->links : nullptr,
                                                            rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1), c->NP, c->nx, c->ny, c->nz,
-                                                           c->zc_tma, om_r, om_b, G, c->diag_cta, T(c->beta), row_split);
+                                                           c->zc_tma, om_r, om_b, G, c->diag_cta, T(c->beta), col_split);
     c->launches += 1;
     CU(cudaGetLastError());
     return LB_OK;
@@ -902,11 +901,11 @@ int step_node(lb_ctx* c) {
     if (rc != LB_OK) return rc;
     auto kern = k_step_node<T, OP_TY>;
     constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
-    int row_split;
-    const dim3 grid(tma_grid(c, true, row_split));
+    int col_split;
+    const dim3 grid(tma_grid(c, true, col_split));
     kern<<<grid, OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                        static_cast<T*>(c->f[c->cur ^ 1]), rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1),
-                                                       c->NP, c->nx, c->ny, c->nz, c->zc_tma, T(1.0 / c->tau[0]), T(1.0 / c->tau[1]), T(c->G), row_split);
+                                                       c->NP, c->nx, c->ny, c->nz, c->zc_tma, T(1.0 / c->tau[0]), T(1.0 / c->tau[1]), T(c->G), col_split);
     c->launches += 1;
     CU(cudaGetLastError());
     c->cur ^= 1;

@@ -19,7 +19,7 @@ template <typename T, int TY>
 __global__ void __launch_bounds__(32 * TY + 128, 1)
 k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
             const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g,
-            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G, int row_split = 1 << 30) {
+            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G, int col_split = 1 << 30) {
     using L = TmaLayout<T, TY>;
     constexpr int TX = L::TX, NT = L::NT, NC = NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     constexpr bool HAS_SOLID = false;
@@ -46,7 +46,7 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
     const int btx = blockIdx.x, bty = blockIdx.y;
     const int x0 = btx * TX, y0 = bty * TY;
     int z0, niter_cta;
-    if (!chunk_range(bty, row_split, nz, zc, z0, niter_cta)) return;
+    if (!chunk_range(bty * ntx + btx, col_split, nz, zc, z0, niter_cta)) return;
     // The iteration count differs between CTAs: it lives in shared memory and is re-read where it is used (a register held across
     // the plane loop costs the consumers a spill: +9 local loads per plane, 3.5 % of the step).
     int* const niter_slot = reinterpret_cast<int*>(sm + L::CST + 8);

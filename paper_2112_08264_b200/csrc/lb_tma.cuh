@@ -147,13 +147,14 @@ struct TmaLayout {
 
 
 // ---- which z chunk a CTA takes ---------------------------------------------------------------------------------
-// Grid (ntx, nty, chunks).  Tile rows bty < row_split are cut into nz / zc chunks of zc planes; the rows from row_split on (the
-// host picks how many, so that the number of working CTAs is a multiple of the SM count: one CTA per SM, and a last wave that
-// leaves a third of the SMs idle costs more than it looks) into one chunk more, of nz / (nz / zc + 1) planes or one more; the
-// grid then has one more z layer, in which only those rows work.  Returns false for a CTA without work; niter = planes + 2.
-__device__ __forceinline__ bool chunk_range(int bty, int row_split, int nz, int zc, int& z0, int& niter) {
+// Grid (ntx, nty, chunks).  Tile columns col = bty ntx + btx < col_split are cut into nz / zc chunks of zc planes; the columns from
+// col_split on (the host picks how many, so that the number of working CTAs is a multiple of the SM count: one CTA per SM, and a
+// last wave that leaves a third of the SMs idle costs more than it looks) into one chunk more, of nz / (nz / zc + 1) planes or one
+// more; the grid then has one more z layer, in which only those columns work.  Returns false for a CTA without work; niter =
+// planes + 2.
+__device__ __forceinline__ bool chunk_range(int col, int col_split, int nz, int zc, int& z0, int& niter) {
     const int c = blockIdx.z;
-    if (bty < row_split) {
+    if (col < col_split) {
         if (c * zc >= nz) return false;
         z0 = c * zc;
         niter = zc + 2;
@@ -182,7 +183,7 @@ __global__ void __launch_bounds__(2 * 32 * TY + 128, 1)
 k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
            const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g, const unsigned* __restrict__ links,
            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc,
-           T om_r, T om_b, T G, double* __restrict__ diag_part = nullptr, T beta = T(0), int row_split = 1 << 30) {
+           T om_r, T om_b, T G, double* __restrict__ diag_part = nullptr, T beta = T(0), int col_split = 1 << 30) {
     static_assert(!(DIAG && HAS_SOLID), "the fused sums assume periodic streaming without bounce-back");
     static_assert(!(MODEL != 0 && (HAS_SOLID || DIAG)), "the colour-gradient variant is built for boxes without solids, without fused sums");
     using L = TmaLayout<T, TY>;
@@ -208,7 +209,7 @@ k_step_tma(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUt
     const int btx = blockIdx.x, bty = blockIdx.y;
     const int x0 = btx * TX, y0 = bty * TY;
     int z0, niter_cta;                        // planes z0-1 .. z0+niter-2; the first and the last are re-collided only
-    if (!chunk_range(bty, row_split, nz, zc, z0, niter_cta)) return;   // (the host guarantees nz % zc == 0)
+    if (!chunk_range(bty * ntx + btx, col_split, nz, zc, z0, niter_cta)) return;   // (the host guarantees nz % zc == 0)
     // The iteration count differs between CTAs: it lives in shared memory and is re-read where it is used (a register held across
     // the plane loop costs the consumers a spill: +9 local loads per plane, 3.5 % of the step).
     int* const niter_slot = reinterpret_cast<int*>(sm + L::CST + 8);
