@@ -394,6 +394,8 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
         box.set_option(B.LB_OPT_DIAG, 1)
     if args.zc:
         box.set_option(B.LB_OPT_ZC, args.zc)
+    if args.no_balance:
+        box.set_option(B.LB_OPT_BALANCE, 0)
     if args.model == "cg":                       # the paper's own two-fluid operator, general two-pass path
         box.set_colour_gradient(args.sigma, args.beta)
     if mask is not None and args.moving_walls:   # prescribed sphere velocities + force / torque per sphere (N2), same path
@@ -531,6 +533,7 @@ def main():
     ap.add_argument("--f32", action="store_true", help="run the workload in fp32 (e.g. config1 --f32 --model cg: the paper's Table 2 setting)")
     ap.add_argument("--decomposition", default="replicas", choices=["replicas", "slab"],
                     help="--gpus N: N independent replicas (north_star: the path does not shard) or ONE box in N z slabs with halo exchange (N3)")
+    ap.add_argument("--no-balance", action="store_true", help="LB_OPT_BALANCE = 0: no padding of the CTA count to whole waves (A/B)")
     ap.add_argument("--zc", type=int, default=0, help="planes per CTA of the one-pass kernels (LB_OPT_ZC); 0 = the library's heuristic")
     ap.add_argument("--diag", action="store_true", help="per-step mass / momentum sums fused into the step kernel (LB_OPT_DIAG)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "twopass", "onepass", "tma", "halo", "node"])

@@ -17,7 +17,7 @@ import numpy as np
 LB_OK, LB_EINVAL, LB_ENOMEM, LB_ECUDA, LB_ESTATE = 0, -1, -2, -3, -4
 LB_F64, LB_F32 = 0, 1
 LB_KERNEL_AUTO, LB_KERNEL_TWOPASS, LB_KERNEL_ONEPASS, LB_KERNEL_TMA, LB_KERNEL_HALO, LB_KERNEL_NODE = 0, 1, 2, 3, 4, 5
-LB_OPT_ZC, LB_OPT_DIAG = 1, 2
+LB_OPT_ZC, LB_OPT_DIAG, LB_OPT_BALANCE = 1, 2, 3
 LB_MODEL_SHAN_CHEN, LB_MODEL_COLOUR_GRADIENT = 0, 1
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

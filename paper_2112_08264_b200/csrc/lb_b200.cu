@@ -82,7 +82,7 @@ struct lb_ctx {
     int zc_req;        // lb_set_option(LB_OPT_ZC): planes per CTA of the one-pass kernels, 0 = heuristic
     double* diag_part; // [DIAG_BLOCKS][5]
     double* diag_out;  // [5]
-    bool balance;      // tma_grid: pad the CTA count to a multiple of the SM count (LB_BALANCE=0 in the environment switches it off: experiments)
+    bool balance;      // tma_grid: pad the CTA count to a multiple of the SM count (LB_OPT_BALANCE)
     double* na_scratch; // device address of g_noalloc_scratch on this context's device (lb_diagnostics_noalloc), nullptr if unknown
     long long launches;
 };
@@ -1214,7 +1214,7 @@ lb_ctx* lb_create_ex(int nx, int ny, int nz, double tau_r, double tau_b, double 
         return nullptr;                                  // LB_ECUDA, message set
     }
     c->have_tmap = onepass_ok(c) && make_tmaps(c);
-    { const char* e_ = getenv("LB_BALANCE"); c->balance = !(e_ && e_[0] == '0'); }
+    c->balance = true;
     c->na_scratch = noalloc_scratch_address(c->device);  // set-up for lb_diagnostics_noalloc; a failure is reported there
     c->kernel_req = LB_KERNEL_AUTO;
     c->kernel = resolve_kernel(c, LB_KERNEL_AUTO);
@@ -1268,6 +1268,10 @@ int lb_set_option(lb_ctx* c, int option, long long value) {
         c->diag_mode = int(value);
         c->diag_fresh = false;
         return LB_OK;
+    case LB_OPT_BALANCE:
+        if (value != 0 && value != 1) return fail(LB_EINVAL, "LB_OPT_BALANCE: 0 or 1");
+        c->balance = value != 0;
+        return LB_OK;
     default:
         return fail(LB_EINVAL, "unknown option");
     }
@@ -1278,6 +1282,7 @@ long long lb_get_option(const lb_ctx* c, int option) {
     switch (option) {
     case LB_OPT_ZC: return (c->kernel == LB_KERNEL_TMA || c->kernel == LB_KERNEL_HALO || c->kernel == LB_KERNEL_NODE) ? tma_zc(c) : c->zc;
     case LB_OPT_DIAG: return c->diag_mode;
+    case LB_OPT_BALANCE: return c->balance ? 1 : 0;
     default: return -1;
     }
 }

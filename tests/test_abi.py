@@ -36,7 +36,7 @@ def test_enums_match_header():
     src = open(os.path.join(ROOT, "include", "lb.h")).read()
     for name in ("LB_OK", "LB_EINVAL", "LB_ENOMEM", "LB_ECUDA", "LB_ESTATE", "LB_F64", "LB_F32",
                  "LB_KERNEL_AUTO", "LB_KERNEL_TWOPASS", "LB_KERNEL_ONEPASS", "LB_KERNEL_TMA", "LB_KERNEL_HALO", "LB_KERNEL_NODE",
-                 "LB_OPT_ZC", "LB_OPT_DIAG", "LB_MODEL_SHAN_CHEN", "LB_MODEL_COLOUR_GRADIENT"):
+                 "LB_OPT_ZC", "LB_OPT_DIAG", "LB_OPT_BALANCE", "LB_MODEL_SHAN_CHEN", "LB_MODEL_COLOUR_GRADIENT"):
         m = re.search(name + r"\s*=\s*(-?\d+)", src)
         assert m and int(m.group(1)) == getattr(B, name), name
 

@@ -648,6 +648,30 @@ def test_state_and_argument_errors():
         assert box.launch_count() > 0
 
 
+@pytest.mark.parametrize("dtype,with_solids", [(B.LB_F64, False), (B.LB_F32, False), (B.LB_F64, True)])
+def test_whole_wave_chunking_changes_no_bit(dtype, with_solids):
+    """LB_OPT_BALANCE (default on) cuts the last tile columns of the TMA-staged kernels into one z chunk more (tma_grid /
+    chunk_range): where the chunk seams lie must not change one bit of the result.  256^3 (1024 CTAs -> 1036 = 7 x 148): every
+    moment of every node after 3 steps, with the option on and off, for k_step_node (fp64), k_step_tma (fp32) and
+    k_step_tma with solid nodes."""
+    cfg = w.CONFIGS[4] if with_solids else w.CONFIGS[1]
+    rr, rb = cfg.fields()
+    mask = cfg.solid_mask() if with_solids else None
+    res = []
+    for balance in (1, 0):
+        with B.Box(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, cfg.G, dtype=dtype) as box:
+            assert box.get_option(B.LB_OPT_BALANCE) == 1         # the default
+            box.set_option(B.LB_OPT_BALANCE, balance)
+            if mask is not None:
+                box.set_solid_mask(mask)
+            box.set_fields(rr, rb)
+            box.step(3)
+            assert B.lb_kernel_name(box.h) == ("tma" if with_solids or dtype == B.LB_F32 else "node")
+            res.append(box.get_moments())
+    for a_, b_ in zip(*res):
+        assert np.array_equal(a_, b_)
+
+
 @pytest.mark.parametrize("kernel", [B.LB_KERNEL_TMA, B.LB_KERNEL_HALO], ids=KNAME.get)
 @pytest.mark.parametrize("dtype,tol_m,tol_p", [(B.LB_F64, 1e-13, 1e-10), (B.LB_F32, 1e-5, 1e-3)])
 def test_fused_per_step_diagnostics_match_oracle(oracle_mod, kernel, dtype, tol_m, tol_p):
