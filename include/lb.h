@@ -144,7 +144,7 @@ int lb_diagnostics_noalloc(lb_ctx* ctx, double* out_dev);
  * LB_KERNEL_TMA instead); LB_KERNEL_AUTO (default) = the TMA-staged pass when the box shape allows
  * it (ONEPASS if the driver cannot encode the tensor maps), else TWOPASS: boxes whose sides are not
  * multiples of the 32 x 8 tile run about 1.5 x slower.  Under AUTO the library picks the thread
- * mapping itself: LB_KERNEL_NODE for an fp64 Shan-Chen box without solid nodes and without
+ * mapping itself: LB_KERNEL_NODE for an fp64 box (either operator) without solid nodes and without
  * LB_OPT_DIAG (measured 0.3 - 1 % faster under the board's power cap), LB_KERNEL_TMA otherwise;
  * lb_get_kernel reports which.  LB_EINVAL if the box shape does not allow `kind`. */
 int lb_set_kernel(lb_ctx* ctx, int kind);
@@ -189,8 +189,9 @@ int lb_last_error_code(void);
 const char* lb_version(void);
 
 /* ---- later operators (the paper's own two-fluid model and its moving walls) -----------------------------------------
- * Colour gradient runs in its own variant of the TMA kernel on boxes without solid nodes that take the 32 x 8 tile
- * (kernel choice AUTO or TMA), everything else (solid nodes, moving walls, other box shapes) on the general two-pass path.
+ * Colour gradient runs in its own variants of the TMA-staged kernels on boxes without solid nodes that take the 32 x 8
+ * tile (kernel choice AUTO, TMA or NODE; AUTO picks NODE in fp64: one colour-blind collision per node instead of one per
+ * component), everything else (solid nodes, moving walls, other box shapes) on the general two-pass path.
  *
  * Colour-gradient collision (Eq. 8-21): replaces the Shan-Chen force + BGK of lb_step by
  *   Theta = (rho^1 - rho^2) / (rho^1 + rho^2), grad Theta = (1 / c_s^2) sum_i w_i Theta(x + c_i) c_i,

@@ -15,15 +15,18 @@
 
 namespace lb {
 
-template <typename T, int TY>
+// MODEL 1: the colour-gradient collision (lb_lattice.cuh collide19_cg_pairs, the MODEL 1 variant of k_step_tma)
+// instead of Shan-Chen force + BGK.  The recolouring works on the colour-blind sum of the two components, which this thread has
+// anyway: one colour-blind collision per node and the two recoloured results, instead of one full collision per component.  The
+// ring holds the phase field Theta; G carries sigma.
+template <typename T, int TY, int MODEL = 0>
 __global__ void __launch_bounds__(32 * TY + 128, 1)
 k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
             const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g,
-            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G, int col_split = 1 << 30) {
+            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G, int col_split = 1 << 30, T beta = T(0)) {
     using L = TmaLayout<T, TY>;
     constexpr int TX = L::TX, NT = L::NT, NC = NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     constexpr bool HAS_SOLID = false;
-    constexpr int MODEL = 0;
     static_assert(TY >= 2 && TY <= 8, "tile rows");
     // register hand-over between the warp groups: (NT + 128) threads start with 65536 / threads registers each
     constexpr int START_REGS = (65536 / (NC + 128)) / 8 * 8;
@@ -58,6 +61,7 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
 
     if (t == 0) {
         niter_slot[0] = niter_cta; niter_slot[1] = z0;
+        sm[L::CST + 5] = T(3) / (T(1) / om_r - T(0.5)); sm[L::CST + 6] = T(3) / (T(1) / om_b - T(0.5));   // 1 / nu_k, nu_k = c_s^2 (tau_k - 1/2)
         for (int s = 0; s < 2; ++s) { mbar_init(full + s, 1); mbar_init(done + s, TY); }
         mbar_init(rdy, 3);
         for (int b = 0; b < 4 * TY; ++b) mbar_init(rowpub + b, 1);
@@ -155,6 +159,14 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
                         if (hxy && mxy == m) v[m] += pxy;
                         if (m < NPOS - 1 || r + m * NR < RS) dst[kk * RS + m * NR] = v[m];
                     }
+                }
+                if (MODEL == 1) {                                           // Theta = (rho^1 - rho^2) / (rho^1 + rho^2), 0 where empty
+#pragma unroll
+                    for (int m = 0; m < NPOS; ++m)
+                        if (m < NPOS - 1 || r + m * NR < RS) {
+                            const T a = dst[m * NR], b = dst[RS + m * NR], sum = a + b;
+                            dst[m * NR] = sum != T(0) ? (a - b) / sum : T(0);
+                        }
                 }
             };
             for (int rp = 0; rp < 2; ++rp) {                                // iteration 0 needs ring planes 0, 1, 2
@@ -268,15 +280,55 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
         __syncwarp();
         if (lane_lo) mbar_arrive(done + sg);            // the producer may refill this stage with the plane after next
 
-        // ---- moments of both components (Eq. 6-7), common velocity (S4) ----
         T rho[2], jx[2], jy[2], jz[2];
+        T ux, uy, uz;
+        T ex[2], ey[2], ez[2];
+        // MODEL 1: rho[k] the densities, jx[0].. the mixture's momentum, ex[0].. grad Theta, and:
+        T cg_rt = zero, cg_x[2] = {zero, zero}, cg_om = zero, cg_amp2 = zero, cg_ig2 = zero, cg_ign = zero, cg_rcs = zero;
+        if constexpr (MODEL == 1) {
+            // the two densities in the order of moments19, the populations summed over the components
+            rho[0] = f[0][0]; rho[1] = f[1][0];
+            f[0][0] += f[1][0];
+#pragma unroll
+            for (int p = 0; p < 9; ++p) {
+                rho[0] += f[0][2 * p + 1] + f[0][2 * p + 2];
+                rho[1] += f[1][2 * p + 1] + f[1][2 * p + 2];
+                f[0][2 * p + 1] += f[1][2 * p + 1]; f[0][2 * p + 2] += f[1][2 * p + 2];
+            }
+            moments19<T>(f[0], cg_rt, jx[0], jy[0], jz[0]);                // rho and rho u of the mixture (Eq. 7)
+            ux = uy = uz = zero;
+            ex[0] = ey[0] = ez[0] = zero;
+            if (cg_rt != zero) {
+                const T irt = T(1) / cg_rt;
+                ux = jx[0] * irt; uy = jy[0] * irt; uz = jz[0] * irt;
+                cg_x[0] = rho[0] * irt; cg_x[1] = rho[1] * irt;
+                const T inv_nu = cg_x[0] * sm[L::CST + 5] + cg_x[1] * sm[L::CST + 6];                 // 1 / nu
+                cg_om = T(2) / (T(6) / inv_nu + T(1));                                             // reading C2
+                // grad Theta = (1 / c_s^2) sum_i w_i Theta(x + c_i) c_i from the ring (reading C1)
+                T d[9];
+#pragma unroll
+                for (int p = 0; p < 9; ++p) {
+                    const int sp = (s0 + pair_cz(p)) & 3, sm_ = (s0 - pair_cz(p)) & 3;
+                    d[p] = w_pair<T>(p) * (ring_n[sp * 2 * RS + pair_cy(p) * RW + pair_cx(p)] - ring_n[sm_ * 2 * RS - pair_cy(p) * RW - pair_cx(p)]);
+                }
+                ex[0] = T(3) * ((((d[0] + d[3]) + d[4]) + d[5]) + d[6]);
+                ey[0] = T(3) * ((((d[1] + d[3]) - d[4]) + d[7]) + d[8]);
+                ez[0] = T(3) * ((((d[2] + d[5]) - d[6]) + d[7]) - d[8]);
+                const T g2 = ex[0] * ex[0] + ey[0] * ey[0] + ez[0] * ez[0];
+                if (g2 != zero) { cg_ig2 = T(1) / g2; cg_ign = T(1) / sqrt(g2); }
+                cg_amp2 = T(2) * (T(0.5) * (T(2.25) * G * cg_om) * (g2 * cg_ign));                 // 2 (A / 2) |grad|, A = (9/4) sigma omega (Eq. 19)
+                cg_rcs = beta * cg_x[0] * cg_x[1] * cg_rt;                                         // beta rho^1 rho^2 / rho (Eq. 20-21)
+            }
+        } else {
+        // ---- moments of both components (Eq. 6-7), common velocity (S4) ----
         moments19<T>(f[0], rho[0], jx[0], jy[0], jz[0]);
         moments19<T>(f[1], rho[1], jx[1], jy[1], jz[1]);
         const T den = om_r * rho[0] + om_b * rho[1];
         const T inv = den != zero ? T(1) / den : zero;
-        const T ux = (om_r * jx[0] + om_b * jx[1]) * inv, uy = (om_r * jy[0] + om_b * jy[1]) * inv, uz = (om_r * jz[0] + om_b * jz[1]) * inv;
+        ux = (om_r * jx[0] + om_b * jx[1]) * inv;
+        uy = (om_r * jy[0] + om_b * jy[1]) * inv;
+        uz = (om_r * jz[0] + om_b * jz[1]) * inv;
         // ---- du^k = -G sum_i w_i rho^kbar(x+c_i) c_i (S2, S3, S6) from the ring ----
-        T ex[2], ey[2], ez[2];
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
             const T* ro_ = ring_n + (1 - k) * RS;
@@ -291,6 +343,7 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
             ez[k] = uz - G * ((((d[2] + d[5]) - d[6]) + d[7]) - d[8]);
         }
 
+        }
         // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) of both components, pair by pair; the stores go out in
         //      plane order (direction-major, the two components adjacent) through one running pointer; the x stage of the density
         //      gather per component as in lb_tma.cuh ----
@@ -298,11 +351,17 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
         T* o = g + (e_own + zl * plu);
         auto put = [&](T v) { st_global(o, v); ptr_step16(o, step16); };
         const T a0 = T(1) - T(1.5) * (ux * ux + uy * uy + uz * uz);
-        T ae[2], wr3[2];
+        T ae[2] = {zero, zero};
+        const T cg_omc = T(1) - cg_om;
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
-            ae[k] = T(1) - T(1.5) * (ex[k] * ex[k] + ey[k] * ey[k] + ez[k] * ez[k]);
-            const T h0 = omc[k] * f[k][0] + w_rest<T>() * rho[k] * (ae[k] - omc[k] * a0);
+            T h0;
+            if constexpr (MODEL == 1) {                                    // cos(phi_0) = 0: no recolouring term
+                h0 = cg_x[k] * (cg_omc * f[0][0] + cg_om * w_rest<T>() * cg_rt * a0 - cg_amp2 * cg_b_rest<T>());
+            } else {
+                ae[k] = T(1) - T(1.5) * (ex[k] * ex[k] + ey[k] * ey[k] + ez[k] * ez[k]);
+                h0 = omc[k] * f[k][0] + w_rest<T>() * rho[k] * (ae[k] - omc[k] * a0);
+            }
             put(h0);
             qb0[k] += h0;
         }
@@ -311,6 +370,16 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
             const T cu = cdot<T>(p, ux, uy, uz);
             const T s0u = a0 + T(4.5) * cu * cu;
             T h1[2], h2[2];
+            if constexpr (MODEL == 1) {                                    // collide19_cg_pairs, once for both components
+                const T cg = cdot<T>(p, ex[0], ey[0], ez[0]);
+                const T wr = cg_om * (w_pair<T>(p) * cg_rt);
+                const T pert = cg_amp2 * (w_pair<T>(p) * cg * cg * cg_ig2 - cg_b_pair<T>(p));             // Eq. 17: the same for i and opp(i)
+                const T recol = cg_rcs * w_pair<T>(p) * cg * cg_ign * (p < 3 ? T(1) : T(0.70710678118654752440));   // cos(phi_i)
+                const T f1 = cg_omc * f[0][2 * p + 1] + wr * (s0u + T(3) * cu) + pert;
+                const T f2 = cg_omc * f[0][2 * p + 2] + wr * (s0u - T(3) * cu) + pert;
+                h1[0] = cg_x[0] * f1 + recol; h2[0] = cg_x[0] * f2 - recol;                               // Eq. 20
+                h1[1] = cg_x[1] * f1 - recol; h2[1] = cg_x[1] * f2 + recol;                               // Eq. 21
+            } else
 #pragma unroll
             for (int k = 0; k < 2; ++k) {
                 const T ce = cdot<T>(p, ex[k], ey[k], ez[k]);

@@ -465,14 +465,14 @@ def _two_phase(nx, ny, nz, seed):
     return rho * (1 + phi) / 2, rho * (1 - phi) / 2, rng.uniform(-0.02, 0.02, (3, nx * ny * nz))
 
 
-@pytest.mark.parametrize("kernel", [B.LB_KERNEL_TMA, B.LB_KERNEL_TWOPASS], ids=KNAME.get)
+@pytest.mark.parametrize("kernel", [B.LB_KERNEL_TMA, B.LB_KERNEL_NODE, B.LB_KERNEL_TWOPASS], ids=KNAME.get)
 @pytest.mark.parametrize("dtype,tol", [(B.LB_F64, 1e-13), (B.LB_F32, 2e-5)])
 @pytest.mark.parametrize("shape,tau,sigma,beta,solid", [((32, 32, 32), (1.0, 1.0), 0.02, 0.7, False), ((40, 24, 12), (0.8, 1.4), 0.01, 0.99, True),
                                                         ((7, 5, 3), (0.7, 0.9), 0.05, 0.3, False), ((64, 16, 8), (0.6, 1.9), 0.0, 0.5, True),
                                                         ((96, 24, 5), (0.8, 1.4), 0.03, 0.9, False), ((64, 16, 6), (0.6, 1.9), 0.01, 0.5, False)])
 def test_colour_gradient_against_oracle(oracle_mod, kernel, dtype, tol, shape, tau, sigma, beta, solid):
-    """Colour gradient on the two-pass path (any box, solids) and in the TMA kernel's own variant (tile-able boxes without solids;
-    with solids the library falls back to the two-pass path whatever the kernel choice)."""
+    """Colour gradient on the two-pass path (any box, solids) and in the TMA-staged kernels' own variants (k_step_tma, k_step_node;
+    tile-able boxes without solids; with solids the library falls back to the two-pass path whatever the kernel choice)."""
     nx, ny, nz = shape
     rr, rb, u = _two_phase(nx, ny, nz, 31)
     mask = None
@@ -490,7 +490,7 @@ def test_colour_gradient_against_oracle(oracle_mod, kernel, dtype, tol, shape, t
         if solid:
             box.set_solid_mask(mask)
         box.set_fields(rr, rb, *u)
-        assert B.lb_kernel_name(box.h) == ("tma" if kernel == B.LB_KERNEL_TMA and not solid else "twopass")
+        assert B.lb_kernel_name(box.h) == (KNAME[kernel] if kernel in (B.LB_KERNEL_TMA, B.LB_KERNEL_NODE) and not solid else "twopass")
         for steps in (1, 4, 25):
             o.step(steps), box.step(steps)
             e = nerr(box.get_populations(), o.get_populations())
@@ -508,7 +508,8 @@ def test_colour_gradient_against_oracle(oracle_mod, kernel, dtype, tol, shape, t
         assert nerr(box.get_populations(), o2.get_populations()) < tol
 
 
-def test_colour_gradient_droplet_256_sampled(oracle_mod):
+@pytest.mark.parametrize("kernel", [B.LB_KERNEL_AUTO, B.LB_KERNEL_TMA, B.LB_KERNEL_NODE], ids=["auto", "tma", "node"])
+def test_colour_gradient_droplet_256_sampled(oracle_mod, kernel):
     """Colour gradient at the paper's box size (256^3, Table 2) from a seeded random colour field: all 38 populations
     at sampled nodes after 6 steps against the oracle on a cut-out (a node depends on the state within 2 nodes per step)."""
     n, s, hw = 256, 6, 13
@@ -518,8 +519,10 @@ def test_colour_gradient_droplet_256_sampled(oracle_mod):
     R, Bl = rr.reshape(n, n, n), rb.reshape(n, n, n)
     with B.Box(n, n, n, 1.0, 1.0, 0.0, dtype=B.LB_F64) as box:
         box.set_colour_gradient(0.02, 0.7)
+        box.set_kernel(kernel)
         box.set_fields(rr, rb)
-        assert B.lb_kernel_name(box.h) == "tma"                  # the colour-gradient variant of the TMA kernel
+        assert B.lb_kernel_name(box.h) in ("tma", "node")        # a colour-gradient variant of the TMA-staged kernels
+        assert kernel == B.LB_KERNEL_AUTO or B.lb_kernel_name(box.h) == KNAME[kernel]
         box.step(s)
         f = box.get_populations()
         for (x, y, z) in rng_nodes:
