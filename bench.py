@@ -473,7 +473,10 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
     alg = ALG_BYTES[cfg.dtype]
     per_launch_ms = ms / max(launches, 1) * (launches / steps)      # = ms / steps: whole step (1 kernel on the one-pass path)
     achieved = alg * N / (per_launch_ms * 1e-3) / 1e9
-    traffic, traffic_src = committed_traffic(cfg.name, kname)
+    # captures are per workload, operator and kernel; a run with other options (moving walls, fused sums, an explicit chunk length)
+    # has no capture of its own
+    plain = not args.moving_walls and not args.diag and not args.zc
+    traffic, traffic_src = committed_traffic(cfg.name + ("_cg" if args.model == "cg" else ""), kname) if plain else (None, None)
     line = {
         "metric": METRIC, "value": glups, "unit": "GLUPS", "n_gpus": world, "steps": steps, "warmup": warmup,
         "ms_per_step": ms_max / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
