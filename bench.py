@@ -434,7 +434,7 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
         m, p = box.get_diagnostics()            # the sums the last step left behind: no population pass
         diag = {"mass": [float(v) for v in m], "momentum": [float(v) for v in p]}
     fused = None
-    if not args.diag and mask is None and args.model == "sc" and (kname in ("tma", "halo") or (kname == "node" and args.kernel == "auto")):
+    if not args.diag and mask is None and args.model == "sc" and kname in ("tma", "halo", "node"):
         # the same K steps once more with the per-step diagnostics fused into the step kernel (LB_OPT_DIAG), for the record
         box.set_option(B.LB_OPT_DIAG, 1)
         box.step(3)

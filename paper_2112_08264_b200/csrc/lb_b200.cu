@@ -900,19 +900,26 @@ int step_node(lb_ctx* c) {
     int rc = ensure_rho<T>(c);
     if (rc != LB_OK) return rc;
     const bool cg = c->model == LB_MODEL_COLOUR_GRADIENT;
-    auto kern = cg ? k_step_node<T, OP_TY, 1> : k_step_node<T, OP_TY, 0>;
+    const bool diag = c->diag_mode && !cg;
+    auto kern = cg ? k_step_node<T, OP_TY, 1, false> : (diag ? k_step_node<T, OP_TY, 0, true> : k_step_node<T, OP_TY, 0, false>);
     constexpr size_t smem = TmaLayout<T, OP_TY>::BYTES;
     int col_split;
-    const dim3 grid(tma_grid(c, true, col_split));
+    const dim3 grid(tma_grid(c, !diag, col_split));
+    if (diag) {
+        const long long ncta = (long long)grid.x * grid.y * grid.z;
+        rc = ensure_diag_buf(c, ncta);
+        if (rc != LB_OK) return rc;
+        c->diag_ncta = ncta;
+    }
     kern<<<grid, OP_TX * OP_TY + 128, smem, c->stream>>>(c->tmap[c->cur][0], c->tmap[c->cur][1], c->tmap[c->cur][2], static_cast<const T*>(c->f[c->cur]),
                                                        static_cast<T*>(c->f[c->cur ^ 1]), rho_view<T>(c, c->rcur), rho_view<T>(c, c->rcur ^ 1),
-                                                       c->NP, c->nx, c->ny, c->nz, c->zc_tma, T(1.0 / c->tau[0]), T(1.0 / c->tau[1]), T(cg ? c->sigma : c->G), col_split, T(c->beta));
+                                                       c->NP, c->nx, c->ny, c->nz, c->zc_tma, T(1.0 / c->tau[0]), T(1.0 / c->tau[1]), T(cg ? c->sigma : c->G), col_split, T(c->beta), c->diag_cta);
     c->launches += 1;
     CU(cudaGetLastError());
     c->cur ^= 1;
     c->rcur ^= 1;
     c->hx_valid = false;
-    c->diag_fresh = false;
+    c->diag_fresh = diag;
     return LB_OK;
 }
 
@@ -1002,6 +1009,7 @@ int configure_onepass_kernels() {
     CU(cudaFuncSetAttribute(k_step_tma<T, false, OP_TY, false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_node<T, OP_TY, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_node<T, OP_TY, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
+    CU(cudaFuncSetAttribute(k_step_node<T, OP_TY, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(TmaLayout<T, OP_TY>::BYTES)));
     CU(cudaFuncSetAttribute(k_step_halo<T, false, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<false>())));
     CU(cudaFuncSetAttribute(k_step_halo<T, true, OP_TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(HaloLayout<T, OP_TY>::template bytes<true>())));
     return LB_OK;
@@ -1060,10 +1068,10 @@ int effective_kernel(const lb_ctx* c) {
     if ((c->kernel == LB_KERNEL_HALO || c->kernel == LB_KERNEL_NODE) && c->has_solid) return LB_KERNEL_TMA;
     // Left to itself (AUTO) a plain fp64 Shan-Chen box runs the one-thread-per-node mapping of the TMA kernel: a third fewer
     // instructions for the same bytes, which under the board's power cap is worth 0.3 % over 20 steps and 1.1 % over 200 at 512^3
-    // (fp32: the (node, component) mapping is 2 % faster).  It has no fused sums: LB_OPT_DIAG keeps k_step_tma.
+    // (fp32: the (node, component) mapping is 2 % faster).
     // The colour gradient gains most from it (one colour-blind collision per node instead of one per component): 256^3 fp64 2.32 ->
     // 2.01 ms, 512^3 17.9 -> 16.3; fp32 the same to 1 % either way.
-    if (c->kernel == LB_KERNEL_TMA && c->kernel_req == LB_KERNEL_AUTO && c->dtype == LB_F64 && !c->has_solid && !c->diag_mode)
+    if (c->kernel == LB_KERNEL_TMA && c->kernel_req == LB_KERNEL_AUTO && c->dtype == LB_F64 && !c->has_solid)
         return LB_KERNEL_NODE;
     return c->kernel;
 }

@@ -19,11 +19,13 @@ namespace lb {
 // instead of Shan-Chen force + BGK.  The recolouring works on the colour-blind sum of the two components, which this thread has
 // anyway: one colour-blind collision per node and the two recoloured results, instead of one full collision per component.  The
 // ring holds the phase field Theta; G carries sigma.
-template <typename T, int TY, int MODEL = 0>
+// DIAG (MODEL 0): the per-component mass and the total momentum of the state after this step, one partial per CTA, as in k_step_tma.
+template <typename T, int TY, int MODEL = 0, bool DIAG = false>
 __global__ void __launch_bounds__(32 * TY + 128, 1)
 k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CUtensorMap tm_w,
             const __grid_constant__ CUtensorMap tm_c, const T* __restrict__ h, T* __restrict__ g,
-            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G, int col_split = 1 << 30, T beta = T(0)) {
+            const RhoView<T> ri, const RhoView<T> ro, long long NP, int nx, int ny, int nz, int zc, T om_r, T om_b, T G, int col_split = 1 << 30, T beta = T(0), double* __restrict__ diag_part = nullptr) {
+    static_assert(!(MODEL != 0 && DIAG), "the fused sums are built for the Shan-Chen step");
     using L = TmaLayout<T, TY>;
     constexpr int TX = L::TX, NT = L::NT, NC = NT, RW = L::RW, RS = L::RS, SUP = L::SUP, W = L::W, PADX = L::PADX;
     constexpr bool HAS_SOLID = false;
@@ -344,6 +346,41 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
         }
 
         }
+        if constexpr (DIAG) {
+            // sum_i f*_i = rho^k and sum_k sum_i f*_i c_i = sum_k (1 - om_k) j^k + rho^k (om_k u' + du^k) (Eq. 1, Eq. 10, S5), which
+            // streaming in a periodic box only permutes; the re-collided planes belong to another chunk
+            double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, v4 = 0.0;
+            if (store_h) {
+                v0 = double(rho[0]); v1 = double(rho[1]);
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    const double oc = double(omc[k]), om = 1.0 - oc, r_ = double(rho[k]);
+                    v2 += oc * double(jx[k]) + r_ * (om * double(ux) + (double(ex[k]) - double(ux)));
+                    v3 += oc * double(jy[k]) + r_ * (om * double(uy) + (double(ey[k]) - double(uy)));
+                    v4 += oc * double(jz[k]) + r_ * (om * double(uz) + (double(ez[k]) - double(uz)));
+                }
+            }
+            // four values, 32 lanes: two halving steps, then three plain ones (lanes 0, 8, 16, 24 end up with the sums of v0..v3);
+            // the fifth by a plain butterfly
+            const bool hA = (tx & 16) != 0, hB = (tx & 8) != 0;
+            double kA = hA ? v2 : v0, kB = hA ? v3 : v1;
+            kA += __shfl_xor_sync(0xffffffffu, hA ? v0 : v2, 16);
+            kB += __shfl_xor_sync(0xffffffffu, hA ? v1 : v3, 16);
+            double kk_ = hB ? kB : kA;
+            kk_ += __shfl_xor_sync(0xffffffffu, hB ? kA : kB, 8);
+            kk_ += __shfl_xor_sync(0xffffffffu, kk_, 4);
+            kk_ += __shfl_xor_sync(0xffffffffu, kk_, 2);
+            kk_ += __shfl_xor_sync(0xffffffffu, kk_, 1);
+#pragma unroll
+            for (int o_ = 16; o_ > 0; o_ >>= 1) v4 += __shfl_xor_sync(0xffffffffu, v4, o_);
+            double* wacc = reinterpret_cast<double*>(smem_tma + L::WACC_BYTE_OFF) + ty * 8;
+            if ((tx & 7) == 0) {
+                double* wa = wacc + (hA ? 2 : 0) + (hB ? 1 : 0);
+                *wa = (it == 0 ? 0.0 : *wa) + kk_;
+            }
+            if (tx == 0) wacc[4] = (it == 0 ? 0.0 : wacc[4]) + v4;
+        }
+
         // ---- BGK collision with exact-difference forcing (Eq. 1, Eq. 10, S5) of both components, pair by pair; the stores go out in
         //      plane order (direction-major, the two components adjacent) through one running pointer; the x stage of the density
         //      gather per component as in lb_tma.cuh ----
@@ -491,6 +528,16 @@ k_step_node(const __grid_constant__ CUtensorMap tm_n, const __grid_constant__ CU
         }
         zt = zl;
         zl = zl + 1 == nz ? 0 : zl + 1;
+    }
+    if constexpr (DIAG) {
+        asm volatile("bar.sync 9, %0;" ::"n"(NC) : "memory");              // every consumer warp's sums are in place
+        if (t < 5) {
+            const double* wp = reinterpret_cast<const double*>(smem_tma + L::WACC_BYTE_OFF);
+            double s_ = 0.0;
+            for (int w_ = 0; w_ < TY; ++w_) s_ += wp[w_ * 8 + t];            // {mass r, mass b, P_x, P_y, P_z}, warps in a fixed order
+            const long long cta = blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z);
+            diag_part[cta * 5 + t] = s_;
+        }
     }
 }
 

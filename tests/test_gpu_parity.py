@@ -13,7 +13,7 @@ from paper_2112_08264_b200 import workloads as w
 pytestmark = pytest.mark.gpu
 
 KERNELS = [B.LB_KERNEL_TWOPASS, B.LB_KERNEL_ONEPASS, B.LB_KERNEL_TMA, B.LB_KERNEL_HALO, B.LB_KERNEL_NODE]
-KNAME = {B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass", B.LB_KERNEL_TMA: "tma", B.LB_KERNEL_HALO: "halo", B.LB_KERNEL_NODE: "node"}
+KNAME = {B.LB_KERNEL_AUTO: "auto", B.LB_KERNEL_TWOPASS: "twopass", B.LB_KERNEL_ONEPASS: "onepass", B.LB_KERNEL_TMA: "tma", B.LB_KERNEL_HALO: "halo", B.LB_KERNEL_NODE: "node"}
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -675,7 +675,7 @@ def test_whole_wave_chunking_changes_no_bit(dtype, with_solids):
         assert np.array_equal(a_, b_)
 
 
-@pytest.mark.parametrize("kernel", [B.LB_KERNEL_TMA, B.LB_KERNEL_HALO], ids=KNAME.get)
+@pytest.mark.parametrize("kernel", [B.LB_KERNEL_TMA, B.LB_KERNEL_HALO, B.LB_KERNEL_NODE, B.LB_KERNEL_AUTO], ids=KNAME.get)
 @pytest.mark.parametrize("dtype,tol_m,tol_p", [(B.LB_F64, 1e-13, 1e-10), (B.LB_F32, 1e-5, 1e-3)])
 def test_fused_per_step_diagnostics_match_oracle(oracle_mod, kernel, dtype, tol_m, tol_p):
     """LB_OPT_DIAG: the TMA / halo step kernel leaves the mass / momentum sums of the NEW state behind (warp shuffles -> per-CTA
