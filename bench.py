@@ -488,6 +488,7 @@ def run_one(args, cfg, B, torch, dev, rank, local_rank, world, cpu_baseline):
                    "parallelism": "replicas only" if world > 1 else "single GPU", "diagnostics_in_step": bool(args.diag),
                    "operator": "colour gradient (sigma %g, beta %g)" % (args.sigma, args.beta) if args.model == "cg" else "Shan-Chen",
                    "moving_walls": bool(mask is not None and args.moving_walls),
+                   "whole_waves": bool(box.get_option(B.LB_OPT_BALANCE)) and not args.zc,
                    **({"note": note} if note else {})},
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                      "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
