@@ -140,7 +140,7 @@ int lb_diagnostics_noalloc(lb_ctx* ctx, double* out_dev);
  * instead of carrying it (less DRAM traffic, measured slower; no bounce-back: a box with solid
  * nodes runs LB_KERNEL_TMA instead); LB_KERNEL_NODE = the TMA-staged single pass with one thread
  * per node doing both components (LB_KERNEL_TMA: one thread per node and component): a third fewer
- * instructions for the same bytes, no bounce-back and no fused sums (a box with solid nodes runs
+ * instructions for the same bytes, no bounce-back (a box with solid nodes runs
  * LB_KERNEL_TMA instead); LB_KERNEL_AUTO (default) = the TMA-staged pass when the box shape allows
  * it (ONEPASS if the driver cannot encode the tensor maps), else TWOPASS: boxes whose sides are not
  * multiples of the 32 x 8 tile run about 1.5 x slower.  Under AUTO the library picks the thread
