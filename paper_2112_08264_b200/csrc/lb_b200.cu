@@ -580,13 +580,32 @@ __global__ void __launch_bounds__(ROW_BX) k_collide_next(const T* __restrict__ h
     if (MOVING && (lk & 0x7FFFEu)) {
         // a loop over the links that exist (few nodes have any, and those few a handful): compact code instead of 18 unrolled copies.
         // The two values of a link are exchanged with the register arrays through a switch-free select chain on the direction.
+        // Force and torque of this node's links are added up in registers and handed to the sphere's sums once per node (the links of a
+        // node nearly always end in one sphere): 6 atomics per node instead of 6 per link.
+        int pcur = -1;
+        double Fa[3] = {0, 0, 0}, Ta[3] = {0, 0, 0};
+        auto flush = [&]() {
+            if (pcur < 0) return;
+#pragma unroll
+            for (int a_ = 0; a_ < 3; ++a_) {
+                if (Fa[a_] != 0.0) atomicAdd(sp.F + 3 * pcur + a_, Fa[a_]);
+                if (Ta[a_] != 0.0) atomicAdd(sp.T + 3 * pcur + a_, Ta[a_]);
+                Fa[a_] = 0.0; Ta[a_] = 0.0;
+            }
+        };
         for (unsigned m = lk & 0x7FFFEu; m; m &= m - 1) {
             const int i = __ffs(int(m)) - 1;
             const int cx = dir_cx(i), cy = dir_cy(i), cz = dir_cz(i);
             const int p = sp.pid[b.at(cx, cy, cz)];
             if (p < 0) continue;
+            if (p != pcur) { flush(); pcur = p; }
             double rbv[3] = {x + 0.5 * cx - sp.c[3 * p], y + 0.5 * cy - sp.c[3 * p + 1], z + 0.5 * cz - sp.c[3 * p + 2]};
-            rbv[0] -= nx * floor(rbv[0] / nx + 0.5); rbv[1] -= ny * floor(rbv[1] / ny + 0.5); rbv[2] -= nz * floor(rbv[2] / nz + 0.5);
+            // minimum image: r - n floor(r / n + 1/2) for |r| < n, without the divisions (this loop runs in most warps: nearly every
+            // 128-node row passes a sphere, and the warp waits for the lane with the most links)
+            const double hx_ = 0.5 * nx, hy_ = 0.5 * ny, hz_ = 0.5 * nz;
+            rbv[0] -= rbv[0] >= hx_ ? double(nx) : (rbv[0] < -hx_ ? -double(nx) : 0.0);
+            rbv[1] -= rbv[1] >= hy_ ? double(ny) : (rbv[1] < -hy_ ? -double(ny) : 0.0);
+            rbv[2] -= rbv[2] >= hz_ ? double(nz) : (rbv[2] < -hz_ ? -double(nz) : 0.0);
             const double ub[3] = {sp.v[3 * p] + (rbv[1] * sp.w[3 * p + 2] - rbv[2] * sp.w[3 * p + 1]),      // Eq. 22 as printed
                                   sp.v[3 * p + 1] + (rbv[2] * sp.w[3 * p] - rbv[0] * sp.w[3 * p + 2]),
                                   sp.v[3 * p + 2] + (rbv[0] * sp.w[3 * p + 1] - rbv[1] * sp.w[3 * p])};
@@ -600,13 +619,12 @@ __global__ void __launch_bounds__(ROW_BX) k_collide_next(const T* __restrict__ h
 #pragma unroll
             for (int q = 1; q < Q; ++q) if (q == i) { fr[q] = br; fb[q] = bb; }
             const double Fv[3] = {mm * cx, mm * cy, mm * cz};
-            if (cx) atomicAdd(sp.F + 3 * p, Fv[0]);
-            if (cy) atomicAdd(sp.F + 3 * p + 1, Fv[1]);
-            if (cz) atomicAdd(sp.F + 3 * p + 2, Fv[2]);
-            atomicAdd(sp.T + 3 * p, Fv[1] * rbv[2] - Fv[2] * rbv[1]);                                 // Eq. 27 as printed: F x r_b
-            atomicAdd(sp.T + 3 * p + 1, Fv[2] * rbv[0] - Fv[0] * rbv[2]);
-            atomicAdd(sp.T + 3 * p + 2, Fv[0] * rbv[1] - Fv[1] * rbv[0]);
+            Fa[0] += Fv[0]; Fa[1] += Fv[1]; Fa[2] += Fv[2];
+            Ta[0] += Fv[1] * rbv[2] - Fv[2] * rbv[1];                                                 // Eq. 27 as printed: F x r_b
+            Ta[1] += Fv[2] * rbv[0] - Fv[0] * rbv[2];
+            Ta[2] += Fv[0] * rbv[1] - Fv[1] * rbv[0];
         }
+        flush();
     }
 #pragma unroll
     for (int i = 0; i < Q; ++i) {
