@@ -651,6 +651,28 @@ def test_state_and_argument_errors():
         assert box.launch_count() > 0
 
 
+@pytest.mark.parametrize("cfg_idx,dtype,model", [(1, B.LB_F64, "sc"), (1, B.LB_F32, "sc"), (4, B.LB_F64, "sc"), (1, B.LB_F64, "cg")])
+def test_run_to_run_determinism_at_bench_size(cfg_idx, dtype, model):
+    """The step kernels have no atomics and no order-dependent sums (single-writer density pieces, fixed-order reductions): two runs of
+    100 steps at 256^3 in the bench launch configuration give the same bits in every moment of every node; a race between CTAs, warps
+    or pipeline stages would show up here."""
+    cfg = w.CONFIGS[cfg_idx]
+    rr, rb = cfg.fields()
+    res = []
+    for _ in range(2):
+        with B.Box(cfg.nx, cfg.ny, cfg.nz, cfg.tau_r, cfg.tau_b, cfg.G if model == "sc" else 0.0, dtype=dtype) as box:
+            if model == "cg":
+                box.set_colour_gradient(0.02, 0.7)
+            if cfg.n_spheres:
+                box.set_solid_mask(cfg.solid_mask())
+            box.set_fields(rr, rb)
+            box.step(100)
+            res.append(box.get_moments())
+    assert all(np.isfinite(a_).all() for a_ in res[0])
+    for a_, b_ in zip(*res):
+        assert np.array_equal(a_, b_)
+
+
 @pytest.mark.parametrize("dtype,with_solids", [(B.LB_F64, False), (B.LB_F32, False), (B.LB_F64, True)])
 def test_whole_wave_chunking_changes_no_bit(dtype, with_solids):
     """LB_OPT_BALANCE (default on) cuts the last tile columns of the TMA-staged kernels into one z chunk more (tma_grid /
